@@ -1,0 +1,426 @@
+/*
+ * tlb_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded fp64 CPU statement of one time step of the 2D thermal
+ * two-component D2Q9 lattice-Boltzmann model of the TLBfind paper (arXiv 2109.12565,
+ * /root/reference/PAPER.md, cited below as "PAPER L<line>").  It exists only so that
+ * tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs can
+ * check and time against it.  It shares no code, header, table or helper with the CUDA
+ * path under paper_2109_12565_b200/ and neither side includes the other.
+ *
+ * The method is an explicit iteration, so the oracle follows it step by step in the
+ * paper's order and notation (PAPER Eqs. (1)-(22)); readings of silent / garbled passages
+ * are the ones listed in DESIGN.md ("Readings R1..R19").  No blocking, fusion or reordering:
+ * every sub-step is a full sweep over the lattice writing a full array.
+ *
+ * Parity pins (tests/test_oracle_pins.py, all run with -m "not gpu"):
+ *   weights            rational invariants of Fig. 1(b)
+ *   bulk update        the paper's printed Table B.8(b) (tests/golden/)
+ *   bounce-back        exact mass conservation, Poiseuille profile            PAPER L151, Eq. (14)
+ *   thermal wall rule  exact linear conduction profile, Nu = 1                PAPER L314, Eq. (24)
+ *   transport coeffs   decay of a shear wave (nu) and of a T mode (kappa)     Eqs. (14), (20)
+ *   forces + pressure  Laplace law on one droplet, flat-interface coexistence Eq. (9)
+ *   buoyancy           barometric density gradient at rest                    Eq. (22)
+ *   posts / corners    second, independently written streaming formulation
+ *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
+ *                      pull of orc_step; beyond that and mass conservation the post-corner
+ *                      rule is a reading (R7/R19): "parity unpinned" for it.
+ *
+ * Build: gcc -O2 -ffp-contract=off -shared -fPIC -o liborc.so tlb_oracle.c -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* ---- D2Q9 lattice, PAPER L74 and Fig. 1(b) L95-102; direction order = reading R1 ---- */
+static const int CX[9] = {0, 1, 0, -1, 0, 1, -1, -1, 1};
+static const int CY[9] = {0, 0, 1, 0, -1, 1, 1, -1, -1};
+static const int OPP[9] = {0, 3, 4, 1, 2, 7, 8, 5, 6};
+static const double W[9] = {4.0 / 9.0,  1.0 / 9.0,  1.0 / 9.0,  1.0 / 9.0, 1.0 / 9.0,
+                            1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0, 1.0 / 36.0};
+
+/* weight p(c) of Fig. 1(b) as a function of |c|^2 (the column printed as "|c_i|") */
+static double p_of_c2(int c2) {
+  switch (c2) {
+    case 0: return 247.0 / 420.0;
+    case 1: return 4.0 / 63.0;
+    case 2: return 4.0 / 135.0;
+    case 4: return 1.0 / 180.0;
+    case 5: return 2.0 / 945.0;
+    case 8: return 1.0 / 15120.0;
+  }
+  return 0.0;
+}
+/* weight w(c) of Fig. 1(b): zero outside the NN zone */
+static double w_of_c2(int c2) {
+  switch (c2) {
+    case 0: return 4.0 / 9.0;
+    case 1: return 1.0 / 9.0;
+    case 2: return 1.0 / 36.0;
+  }
+  return 0.0;
+}
+
+typedef struct orc_params {
+  double tau, tau_g;                  /* Eqs. (2), (16)                       */
+  double rho0;                        /* Eqs. (8), (12)                       */
+  double G12, G11a, G11r, G22a, G22r; /* Eqs. (7), (10), (11)                 */
+  double rho_wall_A, rho_wall_B;      /* rhoWallMax / rhoWallMin, L155        */
+  double T_bottom, T_top, T_ref;      /* Tdown / Tup L314; footnote 3 L182    */
+  double alpha_g;                     /* Eq. (22)                             */
+  double body_ax;                     /* extension: uniform acceleration in x */
+  int32_t periodic_y;                 /* L147, L284-302                       */
+  int32_t thermal;                    /* THERMAL, L314                        */
+} orc_params;
+
+typedef struct orc_state {
+  int nx, ny;
+  orc_params p;
+  double *fA, *fB, *g;       /* [9][ny][nx], time-t populations; 0 on solid sites */
+  double *fAs, *fBs, *gs;    /* post-collision scratch                             */
+  double *rhoA, *rhoB, *T;   /* step 1                                              */
+  double *jx, *jy;           /* step 1                                              */
+  double *psxA, *psxB;       /* psi of Eq. (8)                                      */
+  double *pssA, *pssB;       /* psi of Eq. (12)                                     */
+  double *FAx, *FAy, *FBx, *FBy; /* step 3                                          */
+  double *uHx, *uHy;         /* L139                                                */
+  uint8_t *solid;            /* [ny][nx]                                            */
+} orc_state;
+
+#define IDX(s, x, y) ((size_t)(y) * (size_t)(s)->nx + (size_t)(x))
+#define PIDX(s, i, x, y) ((size_t)(i) * (size_t)(s)->nx * (size_t)(s)->ny + IDX(s, x, y))
+
+static int wrap(int a, int n) {
+  a %= n;
+  return a < 0 ? a + n : a;
+}
+
+/* Is lattice node (x, y) solid?  x is periodic always (L147); y is periodic or bounded by
+ * walls whose first solid rows are y = -1 and y = ny (half-way planes at y = -1/2 and
+ * ny - 1/2); every node beyond a wall is solid (R9). */
+static int is_solid(const orc_state *s, int x, int y) {
+  x = wrap(x, s->nx);
+  if (s->p.periodic_y) y = wrap(y, s->ny);
+  else if (y < 0 || y >= s->ny) return 1;
+  return s->solid[IDX(s, x, y)] != 0;
+}
+
+/* Wall temperature carried by a solid node (R8): bottom half -> T_bottom, top half -> T_top. */
+static double T_wall(const orc_state *s, int y) { return (2 * y < s->ny) ? s->p.T_bottom : s->p.T_top; }
+
+orc_state *orc_create(int nx, int ny, const orc_params *p) {
+  if (nx < 1 || ny < 1 || !p) return NULL;
+  orc_state *s = (orc_state *)calloc(1, sizeof(orc_state));
+  size_t n = (size_t)nx * (size_t)ny;
+  s->nx = nx; s->ny = ny; s->p = *p;
+  double **nine[] = {&s->fA, &s->fB, &s->g, &s->fAs, &s->fBs, &s->gs};
+  for (int k = 0; k < 6; k++) *nine[k] = (double *)calloc(9 * n, sizeof(double));
+  double **one[] = {&s->rhoA, &s->rhoB, &s->T, &s->jx, &s->jy, &s->psxA, &s->psxB, &s->pssA,
+                    &s->pssB, &s->FAx, &s->FAy, &s->FBx, &s->FBy, &s->uHx, &s->uHy};
+  for (int k = 0; k < 15; k++) *one[k] = (double *)calloc(n, sizeof(double));
+  s->solid = (uint8_t *)calloc(n, 1);
+  return s;
+}
+
+void orc_destroy(orc_state *s) {
+  if (!s) return;
+  double *all[] = {s->fA, s->fB, s->g, s->fAs, s->fBs, s->gs, s->rhoA, s->rhoB, s->T, s->jx, s->jy,
+                   s->psxA, s->psxB, s->pssA, s->pssB, s->FAx, s->FAy, s->FBx, s->FBy, s->uHx, s->uHy};
+  for (int k = 0; k < 21; k++) free(all[k]);
+  free(s->solid);
+  free(s);
+}
+
+void orc_set_solid(orc_state *s, const uint8_t *solid) {
+  size_t n = (size_t)s->nx * s->ny;
+  memcpy(s->solid, solid, n);
+  for (int i = 0; i < 9; i++)
+    for (size_t k = 0; k < n; k++)
+      if (s->solid[k]) s->fA[i * n + k] = s->fB[i * n + k] = s->g[i * n + k] = 0.0;
+}
+
+/* Initial populations (R14): equilibrium at rest, f = w rho, g = w T. */
+void orc_set_fields(orc_state *s, const double *rhoA, const double *rhoB, const double *T) {
+  size_t n = (size_t)s->nx * s->ny;
+  for (int i = 0; i < 9; i++)
+    for (size_t k = 0; k < n; k++) {
+      int sol = s->solid[k];
+      s->fA[i * n + k] = sol ? 0.0 : W[i] * rhoA[k];
+      s->fB[i * n + k] = sol ? 0.0 : W[i] * rhoB[k];
+      s->g[i * n + k] = sol ? 0.0 : W[i] * T[k];
+    }
+}
+
+void orc_set_populations(orc_state *s, const double *fA, const double *fB, const double *g) {
+  size_t n9 = 9 * (size_t)s->nx * s->ny;
+  memcpy(s->fA, fA, n9 * sizeof(double));
+  memcpy(s->fB, fB, n9 * sizeof(double));
+  memcpy(s->g, g, n9 * sizeof(double));
+}
+
+void orc_get_populations(const orc_state *s, double *fA, double *fB, double *g) {
+  size_t n9 = 9 * (size_t)s->nx * s->ny;
+  memcpy(fA, s->fA, n9 * sizeof(double));
+  memcpy(fB, s->fB, n9 * sizeof(double));
+  memcpy(g, s->g, n9 * sizeof(double));
+}
+
+/* densities / pseudopotentials seen by the force stencil at ANY node, incl. walls (L155, R9) */
+static double rho_at(const orc_state *s, const double *rho, double rho_wall, int x, int y) {
+  if (is_solid(s, x, y)) return rho_wall;
+  x = wrap(x, s->nx);
+  if (s->p.periodic_y) y = wrap(y, s->ny);
+  return rho[IDX(s, x, y)];
+}
+static double psi_x_of(const orc_state *s, double rho) { return rho / s->p.rho0; }                      /* Eq. (8)  */
+static double psi_s_of(const orc_state *s, double rho) { return s->p.rho0 * (1.0 - exp(-rho / s->p.rho0)); } /* Eq. (12) */
+
+/* Steps 1-4 of the update: moments, pseudopotentials, forces, hydrodynamic velocity.
+ * Everything is a time-t quantity (R13). */
+static void moments_and_forces(orc_state *s) {
+  const int nx = s->nx, ny = s->ny;
+  const orc_params *p = &s->p;
+  /* step 1: Eqs. (4), (5), (17) */
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      size_t k = IDX(s, x, y);
+      if (s->solid[k]) {
+        s->rhoA[k] = p->rho_wall_A; s->rhoB[k] = p->rho_wall_B;
+        s->T[k] = T_wall(s, y); s->jx[k] = s->jy[k] = 0.0;
+        continue;
+      }
+      double ra = 0, rb = 0, t = 0, jx = 0, jy = 0;
+      for (int i = 0; i < 9; i++) {
+        double a = s->fA[PIDX(s, i, x, y)], b = s->fB[PIDX(s, i, x, y)];
+        ra += a; rb += b;
+        jx += CX[i] * a + CX[i] * b;
+        jy += CY[i] * a + CY[i] * b;
+        t += s->g[PIDX(s, i, x, y)];
+      }
+      s->rhoA[k] = ra; s->rhoB[k] = rb; s->T[k] = t; s->jx[k] = jx; s->jy[k] = jy;
+    }
+  /* step 2: Eqs. (8), (12) on every in-domain node (solid nodes hold the wall densities) */
+  for (size_t k = 0; k < (size_t)nx * ny; k++) {
+    s->psxA[k] = psi_x_of(s, s->rhoA[k]); s->psxB[k] = psi_x_of(s, s->rhoB[k]);
+    s->pssA[k] = psi_s_of(s, s->rhoA[k]); s->pssB[k] = psi_s_of(s, s->rhoB[k]);
+  }
+  const double psx_wA = psi_x_of(s, p->rho_wall_A), psx_wB = psi_x_of(s, p->rho_wall_B);
+  const double pss_wA = psi_s_of(s, p->rho_wall_A), pss_wB = psi_s_of(s, p->rho_wall_B);
+  /* step 3: Eqs. (7), (10), (11) then (22) */
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      size_t k = IDX(s, x, y);
+      if (s->solid[k]) { s->FAx[k] = s->FAy[k] = s->FBx[k] = s->FBy[k] = 0; s->uHx[k] = s->uHy[k] = 0; continue; }
+      double xA[2] = {0, 0}, xB[2] = {0, 0}; /* sum_NN w psi^x_{l'}(x+c) c          */
+      double aA[2] = {0, 0}, aB[2] = {0, 0}; /* sum_NN w psi^s_l(x+c) c              */
+      double rA[2] = {0, 0}, rB[2] = {0, 0}; /* sum_{NN+NNN} p psi^s_l(x+c) c        */
+      for (int dy = -2; dy <= 2; dy++)
+        for (int dx = -2; dx <= 2; dx++) {
+          int c2 = dx * dx + dy * dy;
+          if (c2 == 0) continue;
+          int xx = x + dx, yy = y + dy;
+          double nxA, nxB, nsA, nsB;
+          if (is_solid(s, xx, yy)) { nxA = psx_wA; nxB = psx_wB; nsA = pss_wA; nsB = pss_wB; }
+          else {
+            size_t kk = IDX(s, wrap(xx, nx), p->periodic_y ? wrap(yy, ny) : yy);
+            nxA = s->psxA[kk]; nxB = s->psxB[kk]; nsA = s->pssA[kk]; nsB = s->pssB[kk];
+          }
+          double w = w_of_c2(c2), pp = p_of_c2(c2);
+          if (w != 0.0) {
+            xA[0] += w * nxB * dx; xA[1] += w * nxB * dy; /* A feels psi^x of B */
+            xB[0] += w * nxA * dx; xB[1] += w * nxA * dy;
+            aA[0] += w * nsA * dx; aA[1] += w * nsA * dy;
+            aB[0] += w * nsB * dx; aB[1] += w * nsB * dy;
+          }
+          rA[0] += pp * nsA * dx; rA[1] += pp * nsA * dy;
+          rB[0] += pp * nsB * dx; rB[1] += pp * nsB * dy;
+        }
+      double Tk = p->thermal ? s->T[k] : p->T_ref;
+      double FAx = -p->G12 * s->psxA[k] * xA[0] - p->G11a * s->pssA[k] * aA[0] - p->G11r * s->pssA[k] * rA[0];
+      double FAy = -p->G12 * s->psxA[k] * xA[1] - p->G11a * s->pssA[k] * aA[1] - p->G11r * s->pssA[k] * rA[1];
+      double FBx = -p->G12 * s->psxB[k] * xB[0] - p->G22a * s->pssB[k] * aB[0] - p->G22r * s->pssB[k] * rB[0];
+      double FBy = -p->G12 * s->psxB[k] * xB[1] - p->G22a * s->pssB[k] * aB[1] - p->G22r * s->pssB[k] * rB[1];
+      FAy += s->rhoA[k] * p->alpha_g * (Tk - p->T_ref); /* Eq. (22), R12 */
+      FBy += s->rhoB[k] * p->alpha_g * (Tk - p->T_ref);
+      FAx += s->rhoA[k] * p->body_ax;                    /* extension     */
+      FBx += s->rhoB[k] * p->body_ax;
+      s->FAx[k] = FAx; s->FAy[k] = FAy; s->FBx[k] = FBx; s->FBy[k] = FBy;
+      /* L139: rho u^(H) = rho u + F/2 */
+      double rho = s->rhoA[k] + s->rhoB[k];
+      s->uHx[k] = (s->jx[k] + 0.5 * (FAx + FBx)) / rho;
+      s->uHy[k] = (s->jy[k] + 0.5 * (FAy + FBy)) / rho;
+    }
+}
+
+/* Eq. (3) / Eq. (18) with c_s^2 = 1/3 */
+static double equilibrium(int i, double dens, double ux, double uy) {
+  double cu = CX[i] * ux + CY[i] * uy;
+  return W[i] * dens * (1.0 + 3.0 * cu + 4.5 * cu * cu - 1.5 * (ux * ux + uy * uy));
+}
+
+/* step 5: BGK collision, Eqs. (2), (6), (16) */
+static void collide(orc_state *s) {
+  const orc_params *p = &s->p;
+  for (int y = 0; y < s->ny; y++)
+    for (int x = 0; x < s->nx; x++) {
+      size_t k = IDX(s, x, y);
+      if (s->solid[k]) continue;
+      double rho = s->rhoA[k] + s->rhoB[k];
+      double ux = s->jx[k] / rho, uy = s->jy[k] / rho;            /* Eq. (5) */
+      double uAx = ux + p->tau * s->FAx[k] / s->rhoA[k];          /* Eq. (6) */
+      double uAy = uy + p->tau * s->FAy[k] / s->rhoA[k];
+      double uBx = ux + p->tau * s->FBx[k] / s->rhoB[k];
+      double uBy = uy + p->tau * s->FBy[k] / s->rhoB[k];
+      for (int i = 0; i < 9; i++) {
+        size_t q = PIDX(s, i, x, y);
+        s->fAs[q] = s->fA[q] - (s->fA[q] - equilibrium(i, s->rhoA[k], uAx, uAy)) / p->tau;
+        s->fBs[q] = s->fB[q] - (s->fB[q] - equilibrium(i, s->rhoB[k], uBx, uBy)) / p->tau;
+        if (p->thermal)
+          s->gs[q] = s->g[q] - (s->g[q] - equilibrium(i, s->T[k], s->uHx[k], s->uHy[k])) / p->tau_g;
+        else
+          s->gs[q] = s->g[q];
+      }
+    }
+}
+
+/* step 6, link-wise pull: f_i(x,t+1) = f*_i(x - c_i) if that node is fluid, else half-way
+ * bounce-back f*_opp(i)(x) (L151, R7) and anti-bounce-back for g (R8). */
+static void stream_pull(orc_state *s) {
+  const int nx = s->nx, ny = s->ny;
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      if (s->solid[IDX(s, x, y)]) continue;
+      for (int i = 0; i < 9; i++) {
+        int sx = x - CX[i], sy = y - CY[i];
+        size_t q = PIDX(s, i, x, y);
+        if (!is_solid(s, sx, sy)) {
+          size_t src = PIDX(s, i, wrap(sx, nx), s->p.periodic_y ? wrap(sy, ny) : sy);
+          s->fA[q] = s->fAs[src]; s->fB[q] = s->fBs[src];
+          if (s->p.thermal) s->g[q] = s->gs[src];
+        } else {
+          size_t loc = PIDX(s, OPP[i], x, y);
+          s->fA[q] = s->fAs[loc]; s->fB[q] = s->fBs[loc];
+          if (s->p.thermal) {
+            int wy = s->p.periodic_y ? wrap(sy, ny) : sy;
+            s->g[q] = -s->gs[loc] + 2.0 * W[i] * T_wall(s, wy);
+          }
+        }
+      }
+    }
+}
+
+void orc_step(orc_state *s, long n) {
+  for (long t = 0; t < n; t++) {
+    moments_and_forces(s);
+    collide(s);
+    stream_pull(s);
+  }
+}
+
+/* Second, independently written streaming formulation used only to pin the post-corner /
+ * ghost-node logic: push every post-collision population into a lattice padded by one ghost
+ * layer (PAPER footnote 2, L180), fold periodic ghosts back, then let every solid or ghost
+ * node hand each population it received back to the fluid node it came from, reversed. */
+void orc_step_push_ghost(orc_state *s, long n) {
+  const int nx = s->nx, ny = s->ny, px = nx + 2, py = ny + 2;
+  const size_t pn = (size_t)px * py;
+  double *PA = (double *)malloc(9 * pn * sizeof(double));
+  double *PB = (double *)malloc(9 * pn * sizeof(double));
+  double *PG = (double *)malloc(9 * pn * sizeof(double));
+  uint8_t *got = (uint8_t *)malloc(9 * pn);
+  for (long t = 0; t < n; t++) {
+    moments_and_forces(s);
+    collide(s);
+    memset(got, 0, 9 * pn);
+    /* push */
+    for (int y = 0; y < ny; y++)
+      for (int x = 0; x < nx; x++) {
+        if (s->solid[IDX(s, x, y)]) continue;
+        for (int i = 0; i < 9; i++) {
+          size_t d = (size_t)i * pn + (size_t)(y + CY[i] + 1) * px + (size_t)(x + CX[i] + 1);
+          PA[d] = s->fAs[PIDX(s, i, x, y)]; PB[d] = s->fBs[PIDX(s, i, x, y)]; PG[d] = s->gs[PIDX(s, i, x, y)];
+          got[d] = 1;
+        }
+      }
+    /* every padded node, ghost or not, passes on what it received */
+    for (int gy = -1; gy <= ny; gy++)
+      for (int gx = -1; gx <= nx; gx++)
+        for (int i = 0; i < 9; i++) {
+          size_t d = (size_t)i * pn + (size_t)(gy + 1) * px + (size_t)(gx + 1);
+          if (!got[d]) continue;
+          int tx = wrap(gx, nx), ty = gy;
+          if (s->p.periodic_y) ty = wrap(gy, ny);
+          int solid_here = (ty < 0 || ty >= ny) ? 1 : (s->solid[IDX(s, tx, ty)] != 0);
+          if (!solid_here) { /* fluid target (possibly reached through a periodic ghost) */
+            s->fA[PIDX(s, i, tx, ty)] = PA[d]; s->fB[PIDX(s, i, tx, ty)] = PB[d];
+            if (s->p.thermal) s->g[PIDX(s, i, tx, ty)] = PG[d];
+          } else {           /* wall / post: hand back reversed to the sender */
+            int ox = wrap(gx - CX[i], nx), oy = gy - CY[i];
+            if (s->p.periodic_y) oy = wrap(oy, ny);
+            s->fA[PIDX(s, OPP[i], ox, oy)] = PA[d]; s->fB[PIDX(s, OPP[i], ox, oy)] = PB[d];
+            if (s->p.thermal) s->g[PIDX(s, OPP[i], ox, oy)] = -PG[d] + 2.0 * W[i] * T_wall(s, ty);
+          }
+        }
+  }
+  free(PA); free(PB); free(PG); free(got);
+}
+
+/* Hydrodynamic fields at the current time: rho_A, rho_B, u^(H) (2 planes), T.
+ * Solid sites report rho = rho_wall, u = 0, T = that wall's temperature. */
+void orc_fields(orc_state *s, double *rhoA, double *rhoB, double *u, double *T) {
+  size_t n = (size_t)s->nx * s->ny;
+  moments_and_forces(s);
+  memcpy(rhoA, s->rhoA, n * sizeof(double));
+  memcpy(rhoB, s->rhoB, n * sizeof(double));
+  memcpy(u, s->uHx, n * sizeof(double));
+  memcpy(u + n, s->uHy, n * sizeof(double));
+  memcpy(T, s->T, n * sizeof(double));
+}
+
+/* Interaction + external force on each component (for the tests of Eq. (9) / Eq. (22)). */
+void orc_forces(orc_state *s, double *FA, double *FB) {
+  size_t n = (size_t)s->nx * s->ny;
+  moments_and_forces(s);
+  memcpy(FA, s->FAx, n * sizeof(double)); memcpy(FA + n, s->FAy, n * sizeof(double));
+  memcpy(FB, s->FBx, n * sizeof(double)); memcpy(FB + n, s->FBy, n * sizeof(double));
+}
+
+/* Observables: out = {mass_A, mass_B, E, Nu}.
+ *   mass_l = sum over fluid sites of rho_l                                   (north_star)
+ *   E      = (1/N_fluid) sum |u^(H)|^2                                       (L248, R11)
+ *   Nu     = [<u_y^(H) T> - kappa <d_y T>] / (kappa dT / ny)                 (Eq. (24), R10)
+ * with kappa = (tau_g - 1/2)/3 (Eq. (20)), averages over fluid sites, and
+ * d_y T(x,y) = Tface(x,y+1/2) - Tface(x,y-1/2), Tface = mean of the two adjacent rows when the
+ * neighbour is fluid, the wall temperature when it is solid.  long double accumulators. */
+void orc_observables(orc_state *s, double out[4]) {
+  const int nx = s->nx, ny = s->ny;
+  moments_and_forces(s);
+  long double mA = 0, mB = 0, e = 0, uT = 0, dT = 0;
+  long nf = 0;
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      size_t k = IDX(s, x, y);
+      if (s->solid[k]) continue;
+      nf++;
+      mA += s->rhoA[k]; mB += s->rhoB[k];
+      e += s->uHx[k] * s->uHx[k] + s->uHy[k] * s->uHy[k];
+      uT += s->uHy[k] * s->T[k];
+      double up, dn;
+      if (is_solid(s, x, y + 1)) up = T_wall(s, s->p.periodic_y ? wrap(y + 1, ny) : y + 1);
+      else up = 0.5 * (s->T[k] + s->T[IDX(s, x, s->p.periodic_y ? wrap(y + 1, ny) : y + 1)]);
+      if (is_solid(s, x, y - 1)) dn = T_wall(s, s->p.periodic_y ? wrap(y - 1, ny) : y - 1);
+      else dn = 0.5 * (s->T[k] + s->T[IDX(s, x, s->p.periodic_y ? wrap(y - 1, ny) : y - 1)]);
+      dT += up - dn;
+    }
+  double kappa = (s->p.tau_g - 0.5) / 3.0;
+  double DT = s->p.T_bottom - s->p.T_top;
+  out[0] = (double)mA; out[1] = (double)mB;
+  out[2] = nf ? (double)(e / nf) : 0.0;
+  out[3] = (nf && DT != 0.0) ? (double)((uT / nf - kappa * (dT / nf)) / (kappa * DT / ny)) : 0.0;
+}
+
+/* lattice constants exported for the weight-invariant pins */
+double orc_w(int dx, int dy) { return w_of_c2(dx * dx + dy * dy); }
+double orc_p(int dx, int dy) { return p_of_c2(dx * dx + dy * dy); }
+void orc_direction(int i, int *cx, int *cy, int *opp) { *cx = CX[i]; *cy = CY[i]; *opp = OPP[i]; }

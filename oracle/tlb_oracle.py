@@ -1,0 +1,157 @@
+"""ctypes loader for oracle/tlb_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It shares nothing with paper_2109_12565_b200 (the CUDA path) and
+neither imports the other.  All arithmetic lives in tlb_oracle.c; this file only marshals
+numpy arrays (argument meaning follows PAPER.md Eqs. (1)-(22) and DESIGN.md readings).
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tlb_oracle.c")
+_LIB = os.path.join(_HERE, "liborc.so")
+
+
+def build(force=False):
+    """Compile the oracle with gcc (-O2, no FMA contraction, no fast-math)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class OrcParams(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_double) for n in (
+        "tau", "tau_g", "rho0", "G12", "G11a", "G11r", "G22a", "G22r", "rho_wall_A", "rho_wall_B",
+        "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax")] + [
+        ("periodic_y", ctypes.c_int32), ("thermal", ctypes.c_int32)]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        lib.orc_create.restype = ctypes.c_void_p
+        lib.orc_create.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(OrcParams)]
+        lib.orc_destroy.argtypes = [ctypes.c_void_p]
+        lib.orc_set_solid.argtypes = [ctypes.c_void_p, ctypes.c_void_p]
+        lib.orc_set_fields.argtypes = [ctypes.c_void_p, dp, dp, dp]
+        lib.orc_set_populations.argtypes = [ctypes.c_void_p, dp, dp, dp]
+        lib.orc_get_populations.argtypes = [ctypes.c_void_p, dp, dp, dp]
+        lib.orc_step.argtypes = [ctypes.c_void_p, ctypes.c_long]
+        lib.orc_step_push_ghost.argtypes = [ctypes.c_void_p, ctypes.c_long]
+        lib.orc_fields.argtypes = [ctypes.c_void_p, dp, dp, dp, dp]
+        lib.orc_forces.argtypes = [ctypes.c_void_p, dp, dp]
+        lib.orc_observables.argtypes = [ctypes.c_void_p, dp]
+        lib.orc_w.restype = ctypes.c_double
+        lib.orc_w.argtypes = [ctypes.c_int, ctypes.c_int]
+        lib.orc_p.restype = ctypes.c_double
+        lib.orc_p.argtypes = [ctypes.c_int, ctypes.c_int]
+        lib.orc_direction.argtypes = [ctypes.c_int] + [ctypes.POINTER(ctypes.c_int)] * 3
+        _lib = lib
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _c(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+# parameter names understood by Oracle(**params); anything else (init recipe, posts) is ignored
+PARAM_KEYS = [n for n, _ in OrcParams._fields_]
+
+
+class Oracle:
+    """One lattice of nx x ny sites.  Arrays are [ny][nx] (x fastest); populations [9][ny][nx]."""
+
+    def __init__(self, nx, ny, **params):
+        self.lib = _load()
+        self.nx, self.ny = int(nx), int(ny)
+        p = OrcParams()
+        defaults = dict(tau=1.0, tau_g=1.0, rho0=1.0, G12=0.0, G11a=0.0, G11r=0.0, G22a=0.0, G22r=0.0,
+                        rho_wall_A=0.0, rho_wall_B=0.0, T_bottom=0.0, T_top=0.0, T_ref=0.0, alpha_g=0.0,
+                        body_ax=0.0, periodic_y=0, thermal=1)
+        for k in PARAM_KEYS:
+            setattr(p, k, params.get(k, defaults[k]))
+        self.params = p
+        self.h = self.lib.orc_create(self.nx, self.ny, ctypes.byref(p))
+        if not self.h:
+            raise ValueError("orc_create failed")
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.lib.orc_destroy(self.h)
+            self.h = None
+
+    def set_solid(self, solid):
+        s = np.ascontiguousarray(solid, dtype=np.uint8)
+        assert s.shape == (self.ny, self.nx)
+        self.lib.orc_set_solid(self.h, s.ctypes.data)
+
+    def set_fields(self, rhoA, rhoB, T):
+        a, b, t = _c(rhoA), _c(rhoB), _c(T)
+        assert a.shape == b.shape == t.shape == (self.ny, self.nx)
+        self.lib.orc_set_fields(self.h, _dp(a), _dp(b), _dp(t))
+
+    def set_populations(self, fA, fB, g):
+        a, b, c = _c(fA), _c(fB), _c(g)
+        assert a.shape == (9, self.ny, self.nx)
+        self.lib.orc_set_populations(self.h, _dp(a), _dp(b), _dp(c))
+
+    def get_populations(self):
+        out = [np.empty((9, self.ny, self.nx)) for _ in range(3)]
+        self.lib.orc_get_populations(self.h, *[_dp(o) for o in out])
+        return out
+
+    def step(self, n=1):
+        self.lib.orc_step(self.h, int(n))
+
+    def step_push_ghost(self, n=1):
+        self.lib.orc_step_push_ghost(self.h, int(n))
+
+    def fields(self):
+        rhoA, rhoB, T = (np.empty((self.ny, self.nx)) for _ in range(3))
+        u = np.empty((2, self.ny, self.nx))
+        self.lib.orc_fields(self.h, _dp(rhoA), _dp(rhoB), _dp(u), _dp(T))
+        return rhoA, rhoB, u, T
+
+    def forces(self):
+        FA, FB = np.empty((2, self.ny, self.nx)), np.empty((2, self.ny, self.nx))
+        self.lib.orc_forces(self.h, _dp(FA), _dp(FB))
+        return FA, FB
+
+    def observables(self):
+        out = np.empty(4)
+        self.lib.orc_observables(self.h, _dp(out))
+        return dict(mass_A=out[0], mass_B=out[1], E=out[2], Nu=out[3])
+
+
+def lattice_weights():
+    """(w, p) of Fig. 1(b) as dicts {(dx, dy): weight} over the 5x5 neighbourhood."""
+    lib = _load()
+    w = {(dx, dy): lib.orc_w(dx, dy) for dx in range(-2, 3) for dy in range(-2, 3)}
+    p = {(dx, dy): lib.orc_p(dx, dy) for dx in range(-2, 3) for dy in range(-2, 3)}
+    return w, p
+
+
+def directions():
+    lib = _load()
+    out = []
+    for i in range(9):
+        cx, cy, op = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+        lib.orc_direction(i, ctypes.byref(cx), ctypes.byref(cy), ctypes.byref(op))
+        out.append((cx.value, cy.value, op.value))
+    return out

@@ -1,0 +1,13 @@
+"""B200-native thermal two-component D2Q9 lattice-Boltzmann step (TLBfind, arXiv 2109.12565).
+
+`inputs` (seeded synthetic workloads) imports eagerly; the CUDA binding loads the C-ABI shared
+library on first use and fails loudly if it is missing -- there is no CPU fallback.
+"""
+from . import inputs  # noqa: F401
+
+
+def __getattr__(name):
+    if name in ("TLB", "binding", "load_library", "TLBError", "default_params"):
+        from . import binding
+        return binding if name == "binding" else getattr(binding, name)
+    raise AttributeError(name)
