@@ -1,0 +1,140 @@
+/*
+ * tlb.h -- C ABI of the B200-native thermal two-component D2Q9 lattice-Boltzmann step.
+ *
+ * The operation is the per-time-step update of TLBfind (arXiv 2109.12565); citations are
+ * "PAPER L<line>" into /root/reference/PAPER.md plus the equation / section they fall in.
+ * Readings R1..R19 of silent or garbled passages are listed in DESIGN.md.
+ *
+ * One step (tlb_step) computes, for every fluid site, from time-t populations only (R13):
+ *   moments            rho_l = sum_i f_l,i ; T = sum_i g_i ; j = sum_l,i c_i f_l,i     Eqs. (4),(5),(17) L76-80, L165
+ *   pseudopotentials   psi^x = rho/rho0 ; psi^s = rho0 (1 - exp(-rho/rho0))            Eqs. (8),(12) L114, L131
+ *   forces             cross (NN, w_i), attractive (NN, w_i), repulsive (NN+NNN, p_i)   Eqs. (7),(10),(11) L89, L123-126
+ *   buoyancy           F_l,y += rho_l alpha_g (T - T_ref)                               Eq. (22), footnote L182
+ *   velocities         u = j/rho ; u_l = u + tau F_l/rho_l ; u^(H) = (j + F/2)/rho      Eqs. (5),(6) L78-84; L139
+ *   BGK collision      f_l (rho_l, u_l, tau) ; g (T, u^(H), tau_g)                      Eqs. (2),(3),(16),(18) L67-71, L161-169
+ *   streaming          f_i(x + c_i, t+1) = f*_i(x, t), x periodic                      Eq. (1)
+ *   walls / obstacles  half-way bounce-back for f (L151), anti-bounce-back at the wall
+ *                      temperature for g (L314, R8), wall densities in the force
+ *                      stencil (L155, R9); done by a separate boundary kernel.
+ *
+ * CONVENTIONS
+ *   Lattice: nx x ny sites, x periodic (L147); y bounded by walls whose half-way planes are at
+ *   y = -1/2 and y = ny - 1/2 (API rows y = 0..ny-1 are the paper's fluid rows 1..ny, L155), or
+ *   periodic if params.periodic_y.
+ *   Layout: every field is row-major [ny][nx], x fastest; `u` is [2][ny][nx] (u^(H)_x plane then
+ *   u^(H)_y); a population set is [9][ny][nx] in the direction order (R1)
+ *     i : 0      1      2      3       4       5      6       7        8
+ *     c : (0,0)  (1,0)  (0,1)  (-1,0)  (0,-1)  (1,1)  (-1,1)  (-1,-1)  (1,-1)
+ *   and holds the time-t (post-streaming, pre-collision) populations f_i(x, t); solid sites hold 0.
+ *   Solid sites report rho = rho_wall, u = 0, T = T_bottom in the lower half and T_top in the upper.
+ *   Pointers: every array argument of the un-suffixed calls is a DEVICE pointer owned by the caller;
+ *   the *_host variants take HOST pointers (pinned memory makes the copies asynchronous) and stage
+ *   through the workspace.  Nothing is retained from any argument after the call returns, except
+ *   `workspace` and `stream` given to tlb_create, which must outlive the handle.
+ *   Asynchrony: device-pointer calls enqueue on the handle's stream and return; *_host calls and
+ *   tlb_observables_host return after the stream has been synchronised.
+ *   Errors: every call returns 0 (TLB_OK) or a negative code, never aborts or throws.
+ *   There is no CPU fallback: without a CUDA device tlb_create returns TLB_ECUDA.
+ */
+#ifndef TLB_H
+#define TLB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  TLB_OK = 0,
+  TLB_EINVAL = -1,     /* bad size / parameter / NULL pointer / workspace too small              */
+  TLB_ESTATE = -2,     /* step / fields / observables before any state was set                   */
+  TLB_ECUDA = -3,      /* a CUDA call failed (sticky on the handle); see tlb_last_cuda_error      */
+  TLB_EPLACEMENT = -4  /* tlb_init could not place n_droplets within 1000 * n_droplets candidates */
+};
+
+/* POD, passed by pointer, copied by tlb_create. */
+typedef struct tlb_params {
+  double tau, tau_g;                  /* relaxation times, Eqs. (2),(16); must be > 0.5 (Eqs. (14),(20))   */
+  double rho0;                        /* reference density of Eqs. (8),(12); > 0                            */
+  double G12, G11a, G11r, G22a, G22r; /* couplings of Eqs. (7),(10),(11); G*a < 0 attractive, G*r > 0      */
+  double rho_wall_A, rho_wall_B;      /* densities seen by the force stencil at solid nodes, L155 (R9)      */
+  double T_bottom, T_top, T_ref;      /* wall temperatures L314; buoyancy reference, footnote L182 (R12)    */
+  double alpha_g;                     /* alpha*g of Eq. (22)                                                */
+  double body_ax;                     /* EXTENSION: uniform acceleration along x (Poiseuille test)          */
+  /* input recipe used by tlb_init only */
+  double droplet_radius, min_gap, rho_in, rho_out, noise_amp;
+  int32_t n_droplets;
+  int32_t periodic_y;                 /* 0: walls (default); 1: periodic in y (L147, L284-302)              */
+  int32_t thermal;                    /* THERMAL switch, L314: 0 leaves g untouched and uses T = T_ref      */
+  int32_t post_w, post_h, post_period;/* structured rough walls used by tlb_init (R19); 0,0,0 = smooth      */
+  int32_t pop_precision;              /* 64 (only value accepted in this round)                             */
+  int32_t reserved;
+} tlb_params;
+
+typedef struct tlb_handle tlb_handle;
+
+/* Fill *p with the defaults of BASELINE.json's literal physics (tau = tau_g = 1, rho0 = 1, G12 = 0.405,
+ * G11a = G22a = -9, G11r = G22r = 8.1, rho_wall = 0.52, T_bottom = 1, T_top = 0, T_ref = 0.5,
+ * alpha_g = 1e-4, walls in y, thermal on, no droplets). */
+int tlb_default_params(tlb_params* p);
+
+/* Bytes of device memory tlb_create needs for an nx x ny lattice (both population buffers with
+ * their ghost rows, the solid mask, the boundary-link list, 5 field planes, reduction partials). */
+int tlb_workspace_bytes(int nx, int ny, const tlb_params* p, size_t* bytes);
+
+/* Create a handle on `workspace` (DEVICE pointer, >= tlb_workspace_bytes, 256-byte aligned, caller
+ * owned) that enqueues all work on `stream` (a cudaStream_t passed as void*; NULL = default stream).
+ * TLB_EINVAL: nx, ny < 1, tau or tau_g <= 1/2, rho0 <= 0, posts with periodic_y (the paper's own
+ * warning, footnote L302), 2*post_h >= ny, post_w > post_period, NULL pointers, workspace too small. */
+int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t workspace_bytes,
+               void* stream, tlb_handle** out);
+int tlb_destroy(tlb_handle* h);
+
+/* Seeded initial state of the input recipe: structured posts from params, n_droplets
+ * discs by random sequential addition, +noise, linear T profile (L314), populations at rest
+ * equilibrium f = w rho, g = w T (R14).  Bit-identical to paper_2109_12565_b200/inputs.py. */
+int tlb_init(tlb_handle* h, uint64_t seed);
+
+/* Arbitrary obstacle mask [ny][nx], non-zero = solid (flag field, L286).  Resets the state. */
+int tlb_set_solid(tlb_handle* h, const uint8_t* solid);
+int tlb_set_solid_host(tlb_handle* h, const uint8_t* solid);
+
+/* State from hydrodynamic fields: f_l,i = w_i rho_l, g_i = w_i T at rest (R14); solid sites ignored. */
+int tlb_set_fields(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T);
+int tlb_set_fields_host(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T);
+
+/* State from / to time-t populations, each [9][ny][nx] (checkpoint / restart, L252). */
+int tlb_set_populations(tlb_handle* h, const double* fA, const double* fB, const double* g);
+int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g);
+int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, const double* g);
+int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g);
+
+/* Advance n >= 0 time steps (n = 0 is a no-op): per step one fused force+collide+stream kernel and
+ * one wall/obstacle boundary kernel. */
+int tlb_step(tlb_handle* h, int64_t n);
+
+/* Hydrodynamic fields at the current time: rho_A, rho_B [ny][nx], u = u^(H) [2][ny][nx] (L139),
+ * T [ny][nx].  Any pointer may be NULL to skip that field. */
+int tlb_fields(tlb_handle* h, double* rho_A, double* rho_B, double* u, double* T);
+int tlb_fields_host(tlb_handle* h, double* rho_A, double* rho_B, double* u, double* T);
+
+/* out[4] = { mass_A, mass_B, E, Nu }: mass_l = sum over fluid sites of rho_l (north_star);
+ * E = mean over fluid sites of |u^(H)|^2 (L248, R11); Nu of Eq. (24) L347 in the reading R10.
+ * tlb_observables writes to a DEVICE pointer; tlb_observables_host to a HOST pointer (synchronises).
+ * Deterministic: warp-shuffle block partials combined in a fixed order. */
+int tlb_observables(tlb_handle* h, double* out4);
+int tlb_observables_host(tlb_handle* h, double* out4);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+int64_t tlb_launch_count(const tlb_handle* h);
+
+/* Message for a return code; cudaGetErrorString of the sticky CUDA error of a handle. */
+const char* tlb_error_string(int code);
+const char* tlb_last_cuda_error(const tlb_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TLB_H */

@@ -8,6 +8,7 @@ from . import inputs  # noqa: F401
 
 def __getattr__(name):
     if name in ("TLB", "binding", "load_library", "TLBError", "default_params"):
-        from . import binding
+        import importlib
+        binding = importlib.import_module(__name__ + ".binding")
         return binding if name == "binding" else getattr(binding, name)
     raise AttributeError(name)

@@ -1,0 +1,261 @@
+"""Thin ctypes binding of the C ABI in include/tlb.h (same names, argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch is used for device memory and
+streams.  There is no CPU fallback: if libtlb.so is missing or no CUDA device is present the calls
+raise.  This module never imports anything under oracle/.
+"""
+import ctypes
+import os
+import subprocess
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_CSRC = os.path.join(_HERE, "csrc")
+_INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
+LIB_PATH = os.path.join(_HERE, "libtlb.so")
+SOURCES = ["tlb_step.cu", "tlb_aux.cu", "tlb_api.cu"]
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
+
+TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT = 0, -1, -2, -3, -4
+
+# every symbol include/tlb.h declares
+SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_init", "tlb_set_solid",
+           "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
+           "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step", "tlb_fields",
+           "tlb_fields_host", "tlb_observables", "tlb_observables_host", "tlb_launch_count", "tlb_error_string",
+           "tlb_last_cuda_error"]
+
+
+class TLBParams(ctypes.Structure):
+    """Mirror of `struct tlb_params` (include/tlb.h)."""
+    _fields_ = [(n, ctypes.c_double) for n in (
+        "tau", "tau_g", "rho0", "G12", "G11a", "G11r", "G22a", "G22r", "rho_wall_A", "rho_wall_B",
+        "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax",
+        "droplet_radius", "min_gap", "rho_in", "rho_out", "noise_amp")] + [(n, ctypes.c_int32) for n in (
+            "n_droplets", "periodic_y", "thermal", "post_w", "post_h", "post_period", "pop_precision", "reserved")]
+
+
+class TLBError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("tlb error %d: %s" % (code, msg))
+        self.code = code
+
+
+def _sources_newer():
+    if not os.path.exists(LIB_PATH):
+        return True
+    t = os.path.getmtime(LIB_PATH)
+    deps = [os.path.join(_CSRC, s) for s in SOURCES] + [os.path.join(_CSRC, "tlb_internal.cuh"),
+                                                        os.path.join(_INCLUDE, "tlb.h")]
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def build(force=False, verbose=False):
+    """Compile csrc/*.cu for sm_100a into paper_2109_12565_b200/libtlb.so (in-tree)."""
+    if not force and not _sources_newer():
+        return LIB_PATH
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    tmp = LIB_PATH + ".%d.tmp" % os.getpid()
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", _INCLUDE, "-o", tmp] + \
+          [os.path.join(_CSRC, s) for s in SOURCES]
+    subprocess.check_call(cmd)
+    os.replace(tmp, LIB_PATH)
+    return LIB_PATH
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen libtlb.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise TLBError(TLB_ECUDA, "libtlb.so is not built (run __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, dp, i32, i64 = ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int64
+    pp = ctypes.POINTER(TLBParams)
+    lib.tlb_default_params.argtypes = [pp]
+    lib.tlb_workspace_bytes.argtypes = [i32, i32, pp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.tlb_create.argtypes = [i32, i32, pp, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+    lib.tlb_destroy.argtypes = [vp]
+    lib.tlb_init.argtypes = [vp, ctypes.c_uint64]
+    lib.tlb_set_solid.argtypes = [vp, dp]
+    lib.tlb_set_solid_host.argtypes = [vp, dp]
+    for name in ("tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations", "tlb_get_populations",
+                 "tlb_set_populations_host", "tlb_get_populations_host"):
+        getattr(lib, name).argtypes = [vp, dp, dp, dp]
+    lib.tlb_step.argtypes = [vp, i64]
+    lib.tlb_fields.argtypes = [vp, dp, dp, dp, dp]
+    lib.tlb_fields_host.argtypes = [vp, dp, dp, dp, dp]
+    lib.tlb_observables.argtypes = [vp, dp]
+    lib.tlb_observables_host.argtypes = [vp, dp]
+    lib.tlb_launch_count.argtypes = [vp]
+    lib.tlb_launch_count.restype = i64
+    lib.tlb_error_string.argtypes = [i32]
+    lib.tlb_error_string.restype = ctypes.c_char_p
+    lib.tlb_last_cuda_error.argtypes = [vp]
+    lib.tlb_last_cuda_error.restype = ctypes.c_char_p
+    for name in SYMBOLS:
+        if getattr(lib, name).restype is ctypes.c_int:
+            getattr(lib, name).restype = i32
+    _lib = lib
+    return lib
+
+
+def default_params(**overrides):
+    """tlb_default_params() with keyword overrides; unknown keys raise."""
+    p = TLBParams()
+    load_library().tlb_default_params(ctypes.byref(p))
+    names = {n for n, _ in TLBParams._fields_}
+    for k, v in overrides.items():
+        if k not in names:
+            raise KeyError(k)
+        setattr(p, k, v)
+    return p
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+class TLB:
+    """One lattice on one GPU.  Methods mirror the C calls; tensors are torch CUDA float64 (device
+    variants) or CPU float64 (the *_host variants; pin them for asynchronous copies)."""
+
+    def __init__(self, nx, ny, params=None, device="cuda:0", stream=None, **overrides):
+        import torch
+        self.torch = torch
+        self.lib = load_library()
+        self.nx, self.ny = int(nx), int(ny)
+        self.params = params if params is not None else default_params(**overrides)
+        if params is not None:
+            for k, v in overrides.items():
+                setattr(self.params, k, v)
+        nbytes = ctypes.c_size_t()
+        self._chk(self.lib.tlb_workspace_bytes(self.nx, self.ny, ctypes.byref(self.params), ctypes.byref(nbytes)))
+        if not torch.cuda.is_available():
+            raise TLBError(TLB_ECUDA, "no CUDA device; there is no CPU fallback")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.workspace = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        h = ctypes.c_void_p()
+        self.h = None
+        self._chk(self.lib.tlb_create(self.nx, self.ny, ctypes.byref(self.params), base, nbytes.value,
+                                      self.stream.cuda_stream, ctypes.byref(h)))
+        self.h = h
+
+    def _chk(self, rc):
+        if rc != TLB_OK:
+            msg = self.lib.tlb_error_string(rc).decode()
+            if rc == TLB_ECUDA and getattr(self, "h", None):
+                msg += ": " + self.lib.tlb_last_cuda_error(self.h).decode()
+            raise TLBError(rc, msg)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.tlb_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev(self, t, shape, dtype=None):
+        torch = self.torch
+        dtype = dtype or torch.float64
+        t = torch.as_tensor(t)
+        if t.device != self.device or t.dtype != dtype or not t.is_contiguous():
+            t = t.to(device=self.device, dtype=dtype).contiguous()
+        assert tuple(t.shape) == tuple(shape), (tuple(t.shape), shape)
+        return t
+
+    def _host(self, t, shape, dtype=None):
+        torch = self.torch
+        dtype = dtype or torch.float64
+        t = torch.as_tensor(t)
+        assert t.device.type == "cpu" and t.dtype == dtype and t.is_contiguous() and tuple(t.shape) == tuple(shape)
+        return t
+
+    def _new(self, *shape):
+        return self.torch.empty(shape, dtype=self.torch.float64, device=self.device)
+
+    # ---- the C calls -------------------------------------------------------------------------
+    def init(self, seed):
+        self._chk(self.lib.tlb_init(self.h, int(seed)))
+
+    def set_solid(self, solid):
+        s = self._dev(solid, (self.ny, self.nx), self.torch.uint8)
+        self._chk(self.lib.tlb_set_solid(self.h, s.data_ptr()))
+
+    def set_solid_host(self, solid):
+        s = self._host(solid, (self.ny, self.nx), self.torch.uint8)
+        self._chk(self.lib.tlb_set_solid_host(self.h, s.data_ptr()))
+
+    def set_fields(self, rho_A, rho_B, T):
+        a, b, t = (self._dev(v, (self.ny, self.nx)) for v in (rho_A, rho_B, T))
+        self._chk(self.lib.tlb_set_fields(self.h, a.data_ptr(), b.data_ptr(), t.data_ptr()))
+
+    def set_fields_host(self, rho_A, rho_B, T):
+        a, b, t = (self._host(v, (self.ny, self.nx)) for v in (rho_A, rho_B, T))
+        self._chk(self.lib.tlb_set_fields_host(self.h, a.data_ptr(), b.data_ptr(), t.data_ptr()))
+
+    def set_populations(self, fA, fB, g):
+        a, b, c = (self._dev(v, (9, self.ny, self.nx)) for v in (fA, fB, g))
+        self._chk(self.lib.tlb_set_populations(self.h, a.data_ptr(), b.data_ptr(), c.data_ptr()))
+
+    def get_populations(self):
+        out = [self._new(9, self.ny, self.nx) for _ in range(3)]
+        self._chk(self.lib.tlb_get_populations(self.h, *[o.data_ptr() for o in out]))
+        return out
+
+    def set_populations_host(self, fA, fB, g):
+        a, b, c = (self._host(v, (9, self.ny, self.nx)) for v in (fA, fB, g))
+        self._chk(self.lib.tlb_set_populations_host(self.h, a.data_ptr(), b.data_ptr(), c.data_ptr()))
+
+    def get_populations_host(self, out=None):
+        if out is None:
+            out = [self.torch.empty((9, self.ny, self.nx), dtype=self.torch.float64) for _ in range(3)]
+        a, b, c = (self._host(v, (9, self.ny, self.nx)) for v in out)
+        self._chk(self.lib.tlb_get_populations_host(self.h, a.data_ptr(), b.data_ptr(), c.data_ptr()))
+        return [a, b, c]
+
+    def step(self, n=1):
+        self._chk(self.lib.tlb_step(self.h, int(n)))
+
+    def fields(self):
+        rA, rB, T = self._new(self.ny, self.nx), self._new(self.ny, self.nx), self._new(self.ny, self.nx)
+        u = self._new(2, self.ny, self.nx)
+        self._chk(self.lib.tlb_fields(self.h, rA.data_ptr(), rB.data_ptr(), u.data_ptr(), T.data_ptr()))
+        return rA, rB, u, T
+
+    def fields_host(self, rho_A=None, rho_B=None, u=None, T=None):
+        self._chk(self.lib.tlb_fields_host(self.h, _ptr(rho_A), _ptr(rho_B), _ptr(u), _ptr(T)))
+        return rho_A, rho_B, u, T
+
+    def observables(self):
+        """dict(mass_A, mass_B, E, Nu) read back through tlb_observables_host."""
+        out = (ctypes.c_double * 4)()
+        self._chk(self.lib.tlb_observables_host(self.h, ctypes.cast(out, ctypes.c_void_p)))
+        return dict(mass_A=out[0], mass_B=out[1], E=out[2], Nu=out[3])
+
+    def observables_device(self, out4):
+        self._chk(self.lib.tlb_observables(self.h, out4.data_ptr()))
+        return out4
+
+    def launch_count(self):
+        return int(self.lib.tlb_launch_count(self.h))
+
+
+def params_from_config(cfg):
+    """TLBParams for a workload dict of inputs.config()."""
+    pw, ph, pp = cfg["posts"]
+    kw = dict(cfg["params"])
+    kw.update(cfg["init"])
+    kw.update(post_w=pw, post_h=ph, post_period=pp)
+    return default_params(**kw)

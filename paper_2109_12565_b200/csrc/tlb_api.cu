@@ -1,0 +1,406 @@
+// tlb_api.cu -- the C ABI of include/tlb.h: handle, parameter checks, workspace carving, and the
+// host side of every call (argument marshalling and kernel launches only; no lattice arithmetic).
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "tlb_internal.cuh"
+
+using namespace tlb;
+
+struct tlb_handle {
+  Dev d;
+  tlb_params p;
+  cudaStream_t st;
+  double* S[2];       // population buffers (pull form), 27 planes each
+  double* fld[5];     // rho_A, rho_B, u_x, u_y, T scratch planes
+  uint8_t* solid;
+  int* sites;         // boundary work list
+  int* count;
+  double* partials;
+  double* out4;
+  double* centres;
+  int cur;            // S[cur] holds the current state
+  int n_sites;
+  int seg_rows;
+  bool has_state;
+  cudaError_t err;
+  int64_t launches;
+};
+
+namespace {
+
+size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+struct Layout {
+  size_t S0, S1, fld, solid, sites, count, partials, out4, centres, total;
+};
+
+Layout make_layout(int nx, int ny, const tlb_params* p) {
+  const size_t n = (size_t)nx * ny, plane = (size_t)nx * (ny + 2);
+  Layout L;
+  size_t o = 0;
+  L.S0 = o; o = align_up(o + 27 * plane * sizeof(double));
+  L.S1 = o; o = align_up(o + 27 * plane * sizeof(double));
+  L.fld = o; o = align_up(o + 5 * n * sizeof(double));
+  L.solid = o; o = align_up(o + n);
+  L.sites = o; o = align_up(o + n * sizeof(int));
+  L.count = o; o = align_up(o + sizeof(int));
+  L.partials = o; o = align_up(o + (size_t)kObsBlocks * 8 * sizeof(double));
+  L.out4 = o; o = align_up(o + 4 * sizeof(double));
+  L.centres = o; o = align_up(o + 2 * sizeof(double) * (size_t)(p->n_droplets > 0 ? p->n_droplets : 1));
+  L.total = o;
+  return L;
+}
+
+bool params_ok(int nx, int ny, const tlb_params* p) {
+  if (nx < 1 || ny < 1 || !p) return false;
+  if ((long long)nx * (ny + 2) * 27 >= (1ll << 40)) return false;
+  if ((long long)nx * ny >= (1ll << 31)) return false;
+  if (!(p->tau > 0.5) || !(p->tau_g > 0.5) || !(p->rho0 > 0.0)) return false;
+  if (p->pop_precision != 64 && p->pop_precision != 0) return false;
+  if (p->n_droplets < 0 || p->post_w < 0 || p->post_h < 0 || p->post_period < 0) return false;
+  const bool posts = p->post_w > 0 && p->post_h > 0 && p->post_period > 0;
+  if (posts && (p->periodic_y || 2 * p->post_h >= ny || p->post_w > p->post_period)) return false;
+  return true;
+}
+
+int check(tlb_handle* h) {
+  if (h->err == cudaSuccess) h->err = cudaGetLastError();
+  return h->err == cudaSuccess ? TLB_OK : TLB_ECUDA;
+}
+int cu(tlb_handle* h, cudaError_t e) {
+  if (h->err == cudaSuccess && e != cudaSuccess) h->err = e;
+  return h->err == cudaSuccess ? TLB_OK : TLB_ECUDA;
+}
+
+// After the mask changed: rebuild the boundary work list (count comes back to size the launch).
+int rebuild_links(tlb_handle* h) {
+  h->launches += launch_build_links(h->d, h->sites, h->count, h->st);
+  int c = 0;
+  cu(h, cudaMemcpyAsync(&c, h->count, sizeof(int), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  h->n_sites = c;
+  h->has_state = false;
+  return check(h);
+}
+
+// The state in S[cur] was just written by a scatter: make the other buffer consistent (g planes are
+// never rewritten when thermal = 0).
+int after_state_set(tlb_handle* h) {
+  if (!h->d.thermal) h->launches += launch_copy_g(h->d, h->S[h->cur], h->S[1 - h->cur], h->st);
+  h->has_state = true;
+  return check(h);
+}
+
+// SplitMix64-finaliser counter generator of the input recipe (host copy, for the droplet centres)
+double uniform01_host(uint64_t seed, uint64_t stream, uint64_t k) {
+  uint64_t z = seed + 0x9E3779B97F4A7C15ull * ((stream << 40) + k + 1ull);
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  z = z ^ (z >> 31);
+  return (double)(z >> 11) * (1.0 / 9007199254740992.0);
+}
+
+// Random sequential addition of equal discs, periodic in x.  Candidate k
+// is accepted iff it keeps distance >= 2r + min_gap from every accepted centre; a cell list makes
+// the test O(1).  Returns false if n discs could not be placed within 1000 n candidates.
+bool place_droplets(int nx, int ny, uint64_t seed, const tlb_params& p, std::vector<double>& out) {
+  const int n = p.n_droplets;
+  out.clear();
+  if (n == 0) return true;
+  const double r = p.droplet_radius;
+  const double y_lo = r + 3.0 + (double)p.post_h;
+  const double y_hi = (double)ny - 1.0 - y_lo;
+  if (y_hi < y_lo) return false;
+  const double dmin = 2.0 * r + p.min_gap, dmin2 = dmin * dmin;
+  const double cell = dmin > 1.0 ? dmin : 1.0;
+  int gx = (int)std::floor((double)nx / cell), gy = (int)std::floor((double)ny / cell) + 1;
+  if (gx < 1) gx = 1;
+  const double cwx = (double)nx / gx;  // >= cell, so 3 cells cover dmin (all cells when gx < 3)
+  std::vector<std::vector<int>> grid((size_t)gx * gy);
+  const uint64_t kmax = 1000ull * (uint64_t)n;
+  for (uint64_t k = 0; k < kmax && (int)(out.size() / 2) < n; k++) {
+    const double cxd = uniform01_host(seed, 0, 2 * k) * (double)nx;
+    const double t = uniform01_host(seed, 0, 2 * k + 1) * (y_hi - y_lo);
+    const double cyd = y_lo + t;
+    int ix = (int)(cxd / cwx), iy = (int)(cyd / cell);
+    if (ix >= gx) ix = gx - 1;
+    if (iy >= gy) iy = gy - 1;
+    bool ok = true;
+    for (int dj = -1; dj <= 1 && ok; dj++) {
+      const int jy = iy + dj;
+      if (jy < 0 || jy >= gy) continue;
+      // x cells to look at: the three around ix (periodic), or the whole row when it has < 3 cells
+      const int ncell = gx < 3 ? gx : 3;
+      for (int t = 0; t < ncell && ok; t++) {
+        const int c = gx < 3 ? t : ((ix - 1 + t) % gx + gx) % gx;
+        for (int id : grid[(size_t)jy * gx + c]) {
+          double dx = std::fabs(out[2 * id] - cxd);
+          const double alt = (double)nx - dx;
+          if (alt < dx) dx = alt;
+          const double dy = out[2 * id + 1] - cyd;
+          const double dd = dx * dx;
+          const double ee = dy * dy;
+          if (dd + ee < dmin2) { ok = false; break; }
+        }
+      }
+    }
+    if (!ok) continue;
+    grid[(size_t)iy * gx + ix].push_back((int)(out.size() / 2));
+    out.push_back(cxd);
+    out.push_back(cyd);
+  }
+  return (int)(out.size() / 2) == n;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tlb_default_params(tlb_params* p) {
+  if (!p) return TLB_EINVAL;
+  std::memset(p, 0, sizeof(*p));
+  p->tau = 1.0; p->tau_g = 1.0; p->rho0 = 1.0;
+  p->G12 = 0.405; p->G11a = -9.0; p->G11r = 8.1; p->G22a = -9.0; p->G22r = 8.1;
+  p->rho_wall_A = 0.52; p->rho_wall_B = 0.52;
+  p->T_bottom = 1.0; p->T_top = 0.0; p->T_ref = 0.5; p->alpha_g = 1e-4;
+  p->droplet_radius = 6.0; p->min_gap = 4.0; p->rho_in = 1.0; p->rho_out = 0.04; p->noise_amp = 1e-3;
+  p->thermal = 1; p->pop_precision = 64;
+  return TLB_OK;
+}
+
+int tlb_workspace_bytes(int nx, int ny, const tlb_params* p, size_t* bytes) {
+  if (!bytes || !params_ok(nx, ny, p)) return TLB_EINVAL;
+  *bytes = make_layout(nx, ny, p).total;
+  return TLB_OK;
+}
+
+int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t workspace_bytes, void* stream,
+               tlb_handle** out) {
+  if (!out) return TLB_EINVAL;
+  *out = nullptr;
+  if (!params_ok(nx, ny, p) || !workspace || ((uintptr_t)workspace & 255)) return TLB_EINVAL;
+  const Layout L = make_layout(nx, ny, p);
+  if (workspace_bytes < L.total) return TLB_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return TLB_ECUDA;  // no CPU fallback
+  }
+  tlb_handle* h = new (std::nothrow) tlb_handle();
+  if (!h) return TLB_EINVAL;
+  char* w = static_cast<char*>(workspace);
+  h->p = *p;
+  h->st = static_cast<cudaStream_t>(stream);
+  h->S[0] = reinterpret_cast<double*>(w + L.S0);
+  h->S[1] = reinterpret_cast<double*>(w + L.S1);
+  for (int k = 0; k < 5; k++) h->fld[k] = reinterpret_cast<double*>(w + L.fld) + (size_t)k * nx * ny;
+  h->solid = reinterpret_cast<uint8_t*>(w + L.solid);
+  h->sites = reinterpret_cast<int*>(w + L.sites);
+  h->count = reinterpret_cast<int*>(w + L.count);
+  h->partials = reinterpret_cast<double*>(w + L.partials);
+  h->out4 = reinterpret_cast<double*>(w + L.out4);
+  h->centres = reinterpret_cast<double*>(w + L.centres);
+  Dev& d = h->d;
+  d.nx = nx; d.ny = ny; d.periodic_y = p->periodic_y ? 1 : 0; d.thermal = p->thermal ? 1 : 0;
+  d.plane = (long long)nx * (ny + 2);
+  d.omega = 1.0 / p->tau; d.omega_g = 1.0 / p->tau_g; d.tau = p->tau;
+  d.rho0 = p->rho0; d.inv_rho0 = 1.0 / p->rho0;
+  d.G12 = p->G12; d.G11a = p->G11a; d.G11r = p->G11r; d.G22a = p->G22a; d.G22r = p->G22r;
+  d.rho_wall_A = p->rho_wall_A; d.rho_wall_B = p->rho_wall_B;
+  d.pss_wall_A = p->rho0 * (1.0 - std::exp(-p->rho_wall_A / p->rho0));  // Eq. (12) at the wall density
+  d.pss_wall_B = p->rho0 * (1.0 - std::exp(-p->rho_wall_B / p->rho0));
+  d.T_bottom = p->T_bottom; d.T_top = p->T_top; d.T_ref = p->T_ref; d.alpha_g = p->alpha_g; d.body_ax = p->body_ax;
+  d.solid = h->solid;
+  h->cur = 0; h->n_sites = 0; h->has_state = false; h->err = cudaSuccess; h->launches = 0;
+  // rows per CTA segment: aim at >= 8 CTAs per SM, never below 16 rows (4 warm-up rows per segment)
+  const int strips = (nx + kStripW - 1) / kStripW;
+  int segs = (148 * 8 + strips - 1) / strips;
+  int seg = (ny + segs - 1) / segs;
+  if (seg < 16) seg = 16;
+  if (const char* e = std::getenv("TLB_SEG_ROWS")) { const int v = std::atoi(e); if (v > 0) seg = v; }
+  if (seg > ny) seg = ny;
+  h->seg_rows = seg;
+  cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
+  cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.plane * sizeof(double), h->st));
+  cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.plane * sizeof(double), h->st));
+  if (check(h) != TLB_OK) { delete h; return TLB_ECUDA; }
+  *out = h;
+  return TLB_OK;
+}
+
+int tlb_destroy(tlb_handle* h) {
+  if (!h) return TLB_EINVAL;
+  cudaStreamSynchronize(h->st);
+  delete h;
+  return TLB_OK;
+}
+
+int tlb_init(tlb_handle* h, uint64_t seed) {
+  if (!h) return TLB_EINVAL;
+  std::vector<double> c;
+  if (!place_droplets(h->d.nx, h->d.ny, seed, h->p, c)) return TLB_EPLACEMENT;
+  const int n = (int)(c.size() / 2);
+  if (n > 0) {
+    cu(h, cudaMemcpyAsync(h->centres, c.data(), c.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
+    cu(h, cudaStreamSynchronize(h->st));  // `c` is pageable and dies with this frame
+  }
+  h->launches += launch_init(h->d, h->p, seed, h->centres, n, reinterpret_cast<uint8_t*>(h->fld[2]), h->solid,
+                             h->fld[0], h->fld[1], h->fld[4], h->st);
+  int rc = rebuild_links(h);
+  if (rc != TLB_OK) return rc;
+  h->launches += launch_set_fields(h->d, h->fld[0], h->fld[1], h->fld[4], h->S[h->cur], h->st);
+  return after_state_set(h);
+}
+
+int tlb_set_solid(tlb_handle* h, const uint8_t* solid) {
+  if (!h || !solid) return TLB_EINVAL;
+  cu(h, cudaMemcpyAsync(h->solid, solid, (size_t)h->d.nx * h->d.ny, cudaMemcpyDeviceToDevice, h->st));
+  return rebuild_links(h);
+}
+
+int tlb_set_solid_host(tlb_handle* h, const uint8_t* solid) {
+  if (!h || !solid) return TLB_EINVAL;
+  cu(h, cudaMemcpyAsync(h->solid, solid, (size_t)h->d.nx * h->d.ny, cudaMemcpyHostToDevice, h->st));
+  return rebuild_links(h);
+}
+
+int tlb_set_fields(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T) {
+  if (!h || !rho_A || !rho_B || !T) return TLB_EINVAL;
+  h->launches += launch_set_fields(h->d, rho_A, rho_B, T, h->S[h->cur], h->st);
+  return after_state_set(h);
+}
+
+int tlb_set_fields_host(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T) {
+  if (!h || !rho_A || !rho_B || !T) return TLB_EINVAL;
+  const size_t b = (size_t)h->d.nx * h->d.ny * sizeof(double);
+  cu(h, cudaMemcpyAsync(h->fld[0], rho_A, b, cudaMemcpyHostToDevice, h->st));
+  cu(h, cudaMemcpyAsync(h->fld[1], rho_B, b, cudaMemcpyHostToDevice, h->st));
+  cu(h, cudaMemcpyAsync(h->fld[4], T, b, cudaMemcpyHostToDevice, h->st));
+  h->launches += launch_set_fields(h->d, h->fld[0], h->fld[1], h->fld[4], h->S[h->cur], h->st);
+  int rc = after_state_set(h);
+  cu(h, cudaStreamSynchronize(h->st));
+  return rc != TLB_OK ? rc : check(h);
+}
+
+int tlb_set_populations(tlb_handle* h, const double* fA, const double* fB, const double* g) {
+  if (!h || !fA || !fB || !g) return TLB_EINVAL;
+  h->launches += launch_scatter(h->d, fA, fB, g, h->S[h->cur], h->st);
+  return after_state_set(h);
+}
+
+int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  h->launches += launch_gather(h->d, h->S[h->cur], fA, fB, g, h->st);
+  return check(h);
+}
+
+// Host variants stage [27][ny][nx] through the buffer that is not current (it is rewritten by the
+// next step anyway; its g planes are restored when thermal = 0).
+int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, const double* g) {
+  if (!h || !fA || !fB || !g) return TLB_EINVAL;
+  const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
+  double* stage = h->S[1 - h->cur];
+  cu(h, cudaMemcpyAsync(stage, fA, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
+  cu(h, cudaMemcpyAsync(stage + n9, fB, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
+  cu(h, cudaMemcpyAsync(stage + 2 * n9, g, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
+  h->launches += launch_scatter(h->d, stage, stage + n9, stage + 2 * n9, h->S[h->cur], h->st);
+  // the staging area overlapped ghost / solid entries of the other buffer: they are dead until the
+  // next boundary kernel rewrites them
+  int rc = after_state_set(h);
+  cu(h, cudaStreamSynchronize(h->st));
+  return rc != TLB_OK ? rc : check(h);
+}
+
+int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g) {
+  if (!h || !fA || !fB || !g) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
+  double* stage = h->S[1 - h->cur];
+  h->launches += launch_gather(h->d, h->S[h->cur], stage, stage + n9, stage + 2 * n9, h->st);
+  cu(h, cudaMemcpyAsync(fA, stage, n9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaMemcpyAsync(fB, stage + n9, n9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaMemcpyAsync(g, stage + 2 * n9, n9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  if (!h->d.thermal) h->launches += launch_copy_g(h->d, h->S[h->cur], stage, h->st);
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
+int tlb_step(tlb_handle* h, int64_t n) {
+  if (!h || n < 0) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  if (h->err != cudaSuccess) return TLB_ECUDA;
+  for (int64_t t = 0; t < n; t++) {
+    double* in = h->S[h->cur];
+    double* out = h->S[1 - h->cur];
+    h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);
+    h->launches += launch_boundary(h->d, out, h->sites, h->n_sites, h->st);
+    h->cur = 1 - h->cur;
+  }
+  return check(h);
+}
+
+static int fields_to_scratch(tlb_handle* h) {
+  h->launches += launch_fields(h->d, h->S[h->cur], h->fld[0], h->fld[1], h->fld[2], h->fld[3], h->fld[4], h->st);
+  return check(h);
+}
+
+int tlb_fields(tlb_handle* h, double* rho_A, double* rho_B, double* u, double* T) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  const size_t n = (size_t)h->d.nx * h->d.ny;
+  h->launches += launch_fields(h->d, h->S[h->cur], rho_A, rho_B, u, u ? u + n : nullptr, T, h->st);
+  return check(h);
+}
+
+int tlb_fields_host(tlb_handle* h, double* rho_A, double* rho_B, double* u, double* T) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  const size_t n = (size_t)h->d.nx * h->d.ny, b = n * sizeof(double);
+  fields_to_scratch(h);
+  if (rho_A) cu(h, cudaMemcpyAsync(rho_A, h->fld[0], b, cudaMemcpyDeviceToHost, h->st));
+  if (rho_B) cu(h, cudaMemcpyAsync(rho_B, h->fld[1], b, cudaMemcpyDeviceToHost, h->st));
+  if (u) cu(h, cudaMemcpyAsync(u, h->fld[2], 2 * b, cudaMemcpyDeviceToHost, h->st));
+  if (T) cu(h, cudaMemcpyAsync(T, h->fld[4], b, cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
+int tlb_observables(tlb_handle* h, double* out4) {
+  if (!h || !out4) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  fields_to_scratch(h);
+  h->launches += launch_observables(h->d, h->fld[0], h->fld[1], h->fld[2], h->fld[3], h->fld[4], h->partials,
+                                    kObsBlocks, out4, h->st);
+  return check(h);
+}
+
+int tlb_observables_host(tlb_handle* h, double* out4) {
+  if (!h || !out4) return TLB_EINVAL;
+  int rc = tlb_observables(h, h->out4);
+  if (rc != TLB_OK) return rc;
+  cu(h, cudaMemcpyAsync(out4, h->out4, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
+int64_t tlb_launch_count(const tlb_handle* h) { return h ? h->launches : 0; }
+
+const char* tlb_error_string(int code) {
+  switch (code) {
+    case TLB_OK: return "ok";
+    case TLB_EINVAL: return "invalid argument (size, parameter, NULL pointer or workspace too small)";
+    case TLB_ESTATE: return "no state: call tlb_init, tlb_set_fields or tlb_set_populations first";
+    case TLB_ECUDA: return "CUDA error (see tlb_last_cuda_error); there is no CPU fallback";
+    case TLB_EPLACEMENT: return "tlb_init could not place n_droplets by random sequential addition";
+  }
+  return "unknown error code";
+}
+
+const char* tlb_last_cuda_error(const tlb_handle* h) { return cudaGetErrorString(h ? h->err : cudaSuccess); }
+
+}  // extern "C"
