@@ -1,0 +1,262 @@
+#!/usr/bin/env python
+"""bench.py -- MLUPS / HBM roofline of the fused thermal two-component LB step on B200.
+
+    python bench.py --gpus N --steps K --warmup W [--config 1..5] [--impl reference]
+
+A "step" is one lattice-Boltzmann time step (rows a1-a9 of SURVEY.md section 8: fused
+force+collide+stream kernel + boundary kernel) over the whole lattice of the workload.  Default
+workload: BASELINE.json configs[3], the 4096x2048 headline config (4000 droplets r = 14, 4x4 posts
+period 16 on both walls, thermal + buoyancy, fp64), synthetic seeded input.
+N > 1 (torchrun): every rank advances its own replica of the workload (different seed), no
+data-path collective ("replicas only", DESIGN.md section Multi-GPU); value = all ranks' site updates
+over the max-over-ranks device time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+ALG_BYTES_PER_SITE = 432  # 27 fp64 populations read + 27 written
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md
+
+
+def measured_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic(name):
+    """dram bytes per fused-kernel launch from the committed ncu --set full summary, or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            return json.load(f).get(name)
+    except Exception:
+        return None
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi SM clocks and throttle reasons while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5)
+                self.rows.append([c.strip() for c in out.stdout.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        self.stop_flag = True
+        self.join(timeout=6)
+        mhz = sorted(int(r[0]) for r in self.rows if len(r) >= 6 and r[0].isdigit())
+        mx = [int(r[1]) for r in self.rows if len(r) >= 6 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) >= 6 and r[2 + k] == "Active" for r in self.rows)]
+        return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(mhz)}
+
+
+def time_oracle(cfg, solid, rA, rB, T, steps):
+    """MLUPS of the oracle as it stands, single-threaded, on this host."""
+    from oracle import tlb_oracle
+    tlb_oracle.build()
+    o = tlb_oracle.Oracle(cfg["nx"], cfg["ny"], **cfg["params"])
+    o.set_solid(solid)
+    o.set_fields(rA, rB, T)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return cfg["nx"] * cfg["ny"] * steps / dt / 1e6, dt
+
+
+def slab_of(cfg, rows):
+    """A full-width slab of `rows` rows of the workload (walls, posts, droplets, same physics)."""
+    from paper_2109_12565_b200 import inputs
+    if rows >= cfg["ny"]:
+        return cfg, inputs.make_config_inputs(cfg)
+    c = dict(cfg, ny=rows)
+    dens = cfg["init"]["n_droplets"] / float(cfg["nx"] * cfg["ny"])
+    c["init"] = dict(cfg["init"], n_droplets=max(0, int(dens * cfg["nx"] * rows * 0.8)))
+    try:
+        return c, inputs.make_config_inputs(c)
+    except ValueError:
+        c["init"] = dict(cfg["init"], n_droplets=0)
+        return c, inputs.make_config_inputs(c)
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle itself (this tier has no reference implementation), timed on the
+    host cores, each step a bounded slab of the workload sized so the run ends within minutes."""
+    if rank != 0:
+        return
+    from paper_2109_12565_b200 import inputs
+    cfg = inputs.config(args.config)
+    budget_sites = 90e6  # about 90 s at ~1 MLUPS
+    rows = int(budget_sites / max(1, args.steps + args.warmup) / cfg["nx"])
+    rows = max(2 * cfg["posts"][1] + 8, min(cfg["ny"], rows))
+    c, (solid, rA, rB, T) = slab_of(cfg, rows)
+    from oracle import tlb_oracle
+    tlb_oracle.build()
+    o = tlb_oracle.Oracle(c["nx"], c["ny"], **c["params"])
+    o.set_solid(solid)
+    o.set_fields(rA, rB, T)
+    o.step(args.warmup)
+    t0 = time.perf_counter()
+    o.step(args.steps)
+    dt = time.perf_counter() - t0
+    mlups = c["nx"] * c["ny"] * args.steps / dt / 1e6
+    sample = "%dx%d full-width slab of %s per step (walls, posts, droplets kept)" % (c["nx"], c["ny"], cfg["name"])
+    print(json.dumps({
+        "impl": "reference", "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "sample": sample},
+        "cpu_baseline": {"value": mlups, "unit": "MLUPS", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def run_ours(args, rank, world):
+    import torch
+    import torch.distributed as dist
+    from paper_2109_12565_b200 import binding, inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    torch.cuda.set_device(local)
+    dev = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+    binding.load_library()  # raises if libtlb.so is missing
+    cfg = inputs.config(args.config)
+    nx, ny = cfg["nx"], cfg["ny"]
+    sites = nx * ny
+    t = binding.TLB(nx, ny, params=binding.params_from_config(cfg), device=dev)
+    t.init(cfg["seed"] + 1000 * rank)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps, CUDA events on the launch stream, max over ranks
+    t.step(max(3, args.warmup))
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = t.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(t.stream)
+    t.step(args.steps)
+    e1.record(t.stream)
+    barrier()
+    launches = t.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.summary()
+    if world > 1:
+        mt = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(mt, op=dist.ReduceOp.MAX)
+        ms = float(mt.item())
+    mlups = world * sites * args.steps / ms / 1e3
+
+    # ---- roofline of the dominant (fused) kernel: events around every launch of a short window
+    fused_ms, boundary_ms = t.profile_step(min(args.steps, 200))
+    peak, peak_src = measured_peak()
+    achieved = ALG_BYTES_PER_SITE * sites / fused_ms / 1e6  # GB/s
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": committed_traffic(cfg["name"]), "peak_source": peak_src, "kernel": "tlb::fused_kernel<0>",
+                "kernel_ms": fused_ms, "boundary_kernel_ms": boundary_ms, "alg_bytes_per_launch": ALG_BYTES_PER_SITE * sites,
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "kernel_share_of_step": fused_ms / (fused_ms + boundary_ms)}
+    ob = t.observables()
+    finite = all(v == v and abs(v) != float("inf") for v in ob.values())
+
+    # ---- end to end through the host-buffer ABI: per step H2D of the three input fields from pinned
+    # memory, one LB step, D2H of the four observables
+    solid_h = torch.zeros((ny, nx), dtype=torch.uint8)
+    fa, fb, ft = (torch.empty((ny, nx), dtype=torch.float64).pin_memory() for _ in range(3))
+    t.fields_host(fa, fb, None, ft)
+    e2e_steps = max(3, min(args.steps, 20))
+    for _ in range(2):
+        t.set_fields_host(fa, fb, ft); t.step(1); t.observables()
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        t.set_fields_host(fa, fb, ft)
+        t.step(1)
+        t.observables()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - w0) * 1e3
+    if world > 1:
+        mt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(mt, op=dist.ReduceOp.MAX)
+        e2e_ms = float(mt.item())
+    e2e = {"value": world * sites * e2e_steps / e2e_ms / 1e3, "unit": "MLUPS", "h2d_bytes_per_step": 3 * 8 * sites,
+           "d2h_bytes_per_step": 32, "steps": e2e_steps,
+           "call": "tlb_set_fields_host + tlb_step(1) + tlb_observables_host per step"}
+    del solid_h
+
+    # ---- CPU baseline: the oracle as it stands on this host, rank 0 at N = 1 only
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        rows = min(ny, max(64, int(20e6 / nx / 2)))
+        c, (solid, rA, rB, T) = slab_of(cfg, rows)
+        v, dt = time_oracle(c, solid, rA, rB, T, 2)
+        cpu = {"value": v, "unit": "MLUPS", "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": "2 steps of a %dx%d full-width slab of %s (host has %d cores; the oracle is single-threaded)"
+                         % (c["nx"], c["ny"], cfg["name"], os.cpu_count())}
+
+    if rank == 0:
+        print(json.dumps({
+            "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"], "nx": nx, "ny": ny, "droplets": cfg["init"]["n_droplets"],
+                       "posts": list(cfg["posts"]), "state_bytes": 216 * sites,
+                       "l2": "state (%.2f GB per buffer) exceeds the 126 MB L2; no flush needed" % (216 * sites / 1e9)
+                       if 216 * sites > 4 * 126e6 else "state fits in L2: HBM figures are not meaningful",
+                       "parallelism": "replicas x%d" % world, "finite": finite, "mass_A": ob["mass_A"], "Nu": ob["Nu"]},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "effective_GBs": ALG_BYTES_PER_SITE * mlups / 1e3, "roofline_frac_whole_step": ALG_BYTES_PER_SITE * mlups / 1e3 / peak / world}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", type=int, default=4)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -21,7 +21,8 @@ TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT = 0, -1, -2, -3, -4
 # every symbol include/tlb.h declares
 SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_init", "tlb_set_solid",
            "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
-           "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step", "tlb_fields",
+           "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step",
+           "tlb_profile_step", "tlb_fields",
            "tlb_fields_host", "tlb_observables", "tlb_observables_host", "tlb_launch_count", "tlb_error_string",
            "tlb_last_cuda_error"]
 
@@ -87,6 +88,7 @@ def load_library():
                  "tlb_set_populations_host", "tlb_get_populations_host"):
         getattr(lib, name).argtypes = [vp, dp, dp, dp]
     lib.tlb_step.argtypes = [vp, i64]
+    lib.tlb_profile_step.argtypes = [vp, i64, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]
     lib.tlb_fields.argtypes = [vp, dp, dp, dp, dp]
     lib.tlb_fields_host.argtypes = [vp, dp, dp, dp, dp]
     lib.tlb_observables.argtypes = [vp, dp]
@@ -97,9 +99,6 @@ def load_library():
     lib.tlb_error_string.restype = ctypes.c_char_p
     lib.tlb_last_cuda_error.argtypes = [vp]
     lib.tlb_last_cuda_error.restype = ctypes.c_char_p
-    for name in SYMBOLS:
-        if getattr(lib, name).restype is ctypes.c_int:
-            getattr(lib, name).restype = i32
     _lib = lib
     return lib
 
@@ -227,6 +226,12 @@ class TLB:
 
     def step(self, n=1):
         self._chk(self.lib.tlb_step(self.h, int(n)))
+
+    def profile_step(self, n):
+        """(fused_ms, boundary_ms): average kernel durations over n steps, CUDA events on the stream."""
+        a, b = ctypes.c_double(), ctypes.c_double()
+        self._chk(self.lib.tlb_profile_step(self.h, int(n), ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
 
     def fields(self):
         rA, rB, T = self._new(self.ny, self.nx), self._new(self.ny, self.nx), self._new(self.ny, self.nx)

@@ -344,6 +344,35 @@ int tlb_step(tlb_handle* h, int64_t n) {
   return check(h);
 }
 
+int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundary_ms) {
+  if (!h || n < 1 || n > 4096 || !fused_ms || !boundary_ms) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  if (h->err != cudaSuccess) return TLB_ECUDA;
+  std::vector<cudaEvent_t> ev(3 * (size_t)n);
+  for (auto& e : ev) cu(h, cudaEventCreate(&e));
+  for (int64_t t = 0; t < n; t++) {
+    double* in = h->S[h->cur];
+    double* out = h->S[1 - h->cur];
+    cu(h, cudaEventRecord(ev[3 * t], h->st));
+    h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);
+    cu(h, cudaEventRecord(ev[3 * t + 1], h->st));
+    h->launches += launch_boundary(h->d, out, h->sites, h->n_sites, h->st);
+    cu(h, cudaEventRecord(ev[3 * t + 2], h->st));
+    h->cur = 1 - h->cur;
+  }
+  cu(h, cudaStreamSynchronize(h->st));
+  double a = 0.0, b = 0.0;
+  for (int64_t t = 0; t < n && h->err == cudaSuccess; t++) {
+    float ms = 0.f;
+    cu(h, cudaEventElapsedTime(&ms, ev[3 * t], ev[3 * t + 1])); a += ms;
+    cu(h, cudaEventElapsedTime(&ms, ev[3 * t + 1], ev[3 * t + 2])); b += ms;
+  }
+  for (auto& e : ev) cudaEventDestroy(e);
+  *fused_ms = a / (double)n;
+  *boundary_ms = b / (double)n;
+  return check(h);
+}
+
 static int fields_to_scratch(tlb_handle* h) {
   h->launches += launch_fields(h->d, h->S[h->cur], h->fld[0], h->fld[1], h->fld[2], h->fld[3], h->fld[4], h->st);
   return check(h);
