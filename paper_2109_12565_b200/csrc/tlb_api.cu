@@ -17,6 +17,7 @@ struct tlb_handle {
   double* S[2];       // population buffers (pull form), 27 planes each
   double* fld[5];     // rho_A, rho_B, u_x, u_y, T scratch planes
   uint8_t* solid;
+  uint8_t* solidp;     // padded copy for the fused kernel
   int* sites;         // boundary work list
   int* count;
   double* partials;
@@ -35,17 +36,18 @@ namespace {
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
 struct Layout {
-  size_t S0, S1, fld, solid, sites, count, partials, out4, centres, total;
+  size_t S0, S1, fld, solid, solidp, sites, count, partials, out4, centres, total;
 };
 
 Layout make_layout(int nx, int ny, const tlb_params* p) {
-  const size_t n = (size_t)nx * ny, plane = (size_t)nx * (ny + 2);
+  const size_t n = (size_t)nx * ny, px = (size_t)padded_pitch(nx), plane = px * (ny + 2);
   Layout L;
   size_t o = 0;
   L.S0 = o; o = align_up(o + 27 * plane * sizeof(double));
   L.S1 = o; o = align_up(o + 27 * plane * sizeof(double));
   L.fld = o; o = align_up(o + 5 * n * sizeof(double));
   L.solid = o; o = align_up(o + n);
+  L.solidp = o; o = align_up(o + px * ny);
   L.sites = o; o = align_up(o + n * sizeof(int));
   L.count = o; o = align_up(o + sizeof(int));
   L.partials = o; o = align_up(o + (size_t)kObsBlocks * 8 * sizeof(double));
@@ -57,7 +59,7 @@ Layout make_layout(int nx, int ny, const tlb_params* p) {
 
 bool params_ok(int nx, int ny, const tlb_params* p) {
   if (nx < 1 || ny < 1 || !p) return false;
-  if ((long long)nx * (ny + 2) * 27 >= (1ll << 40)) return false;
+  if ((long long)padded_pitch(nx) * (ny + 2) * 27 >= (1ll << 40)) return false;
   if ((long long)nx * ny >= (1ll << 31)) return false;
   if (!(p->tau > 0.5) || !(p->tau_g > 0.5) || !(p->rho0 > 0.0)) return false;
   if (p->pop_precision != 64 && p->pop_precision != 0) return false;
@@ -78,7 +80,7 @@ int cu(tlb_handle* h, cudaError_t e) {
 
 // After the mask changed: rebuild the boundary work list (count comes back to size the launch).
 int rebuild_links(tlb_handle* h) {
-  h->launches += launch_build_links(h->d, h->sites, h->count, h->st);
+  h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);
   int c = 0;
   cu(h, cudaMemcpyAsync(&c, h->count, sizeof(int), cudaMemcpyDeviceToHost, h->st));
   cu(h, cudaStreamSynchronize(h->st));
@@ -199,6 +201,7 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   h->S[1] = reinterpret_cast<double*>(w + L.S1);
   for (int k = 0; k < 5; k++) h->fld[k] = reinterpret_cast<double*>(w + L.fld) + (size_t)k * nx * ny;
   h->solid = reinterpret_cast<uint8_t*>(w + L.solid);
+  h->solidp = reinterpret_cast<uint8_t*>(w + L.solidp);
   h->sites = reinterpret_cast<int*>(w + L.sites);
   h->count = reinterpret_cast<int*>(w + L.count);
   h->partials = reinterpret_cast<double*>(w + L.partials);
@@ -206,7 +209,8 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   h->centres = reinterpret_cast<double*>(w + L.centres);
   Dev& d = h->d;
   d.nx = nx; d.ny = ny; d.periodic_y = p->periodic_y ? 1 : 0; d.thermal = p->thermal ? 1 : 0;
-  d.plane = (long long)nx * (ny + 2);
+  d.px = padded_pitch(nx);
+  d.plane = (long long)d.px * (ny + 2);
   d.omega = 1.0 / p->tau; d.omega_g = 1.0 / p->tau_g; d.tau = p->tau;
   d.rho0 = p->rho0; d.inv_rho0 = 1.0 / p->rho0;
   d.G12 = p->G12; d.G11a = p->G11a; d.G11r = p->G11r; d.G22a = p->G22a; d.G22r = p->G22r;
@@ -215,16 +219,15 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   d.pss_wall_B = p->rho0 * (1.0 - std::exp(-p->rho_wall_B / p->rho0));
   d.T_bottom = p->T_bottom; d.T_top = p->T_top; d.T_ref = p->T_ref; d.alpha_g = p->alpha_g; d.body_ax = p->body_ax;
   d.solid = h->solid;
+  d.solidp = h->solidp;
   h->cur = 0; h->n_sites = 0; h->has_state = false; h->err = cudaSuccess; h->launches = 0;
-  // rows per CTA segment: aim at >= 8 CTAs per SM, never below 16 rows (4 warm-up rows per segment)
-  const int strips = (nx + kStripW - 1) / kStripW;
-  int segs = (148 * 8 + strips - 1) / strips;
-  int seg = (ny + segs - 1) / segs;
-  if (seg < 16) seg = 16;
+  int seg = default_seg_rows(nx, ny);
   if (const char* e = std::getenv("TLB_SEG_ROWS")) { const int v = std::atoi(e); if (v > 0) seg = v; }
   if (seg > ny) seg = ny;
   h->seg_rows = seg;
+  if (configure_kernels() != 0) { cudaGetLastError(); delete h; return TLB_ECUDA; }
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
+  h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field
   cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.plane * sizeof(double), h->st));
   cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.plane * sizeof(double), h->st));
   if (check(h) != TLB_OK) { delete h; return TLB_ECUDA; }

@@ -15,16 +15,20 @@ __device__ __forceinline__ bool fluid_at(const Dev& d, int x, int y) {
   return d.solid[(size_t)y * d.nx + x] == 0;
 }
 
-// One thread per node of the padded lattice (rows -1..ny).  S_i(s) = f_i(s + c_i) when s + c_i is a
-// fluid site (Eq. (1) read backwards), else 0.  RHO = true: f_i = w_i * field (R14).
+// One thread per node of the padded lattice (rows -1..ny, columns -kGhost..nx+kGhost-1; ghost columns
+// are the periodic images).  S_i(s) = f_i(s + c_i) when s + c_i is a fluid site (Eq. (1) read
+// backwards), else 0.  RHO = true: f_i = w_i * field (R14).
 template <bool RHO>
 __global__ void scatter_kernel(const Dev d, const double* __restrict__ a, const double* __restrict__ b,
                                const double* __restrict__ c, double* __restrict__ S) {
+  const int nx = d.nx, ny = d.ny, wpad = nx + 2 * kGhost;
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= d.plane) return;
-  const int nx = d.nx, ny = d.ny;
-  const int sx = (int)(k % nx), sy = (int)(k / nx) - 1;
+  if (k >= (long long)wpad * (ny + 2)) return;
+  const int gx = (int)(k % wpad) - kGhost, sy = (int)(k / wpad) - 1;
+  int sx = gx % nx;
+  if (sx < 0) sx += nx;
   const size_t n = (size_t)nx * ny;
+  const long long o = d.at(gx, sy);
 #pragma unroll
   for (int i = 0; i < 9; i++) {
     const int x = wrapi(sx + cx(i), nx);
@@ -40,9 +44,9 @@ __global__ void scatter_kernel(const Dev d, const double* __restrict__ a, const 
         va = a[i * n + q]; vb = b[i * n + q]; vc = c[i * n + q];
       }
     }
-    S[i * d.plane + k] = va;
-    S[(9 + i) * d.plane + k] = vb;
-    S[(18 + i) * d.plane + k] = vc;
+    S[i * d.plane + o] = va;
+    S[(9 + i) * d.plane + o] = vb;
+    S[(18 + i) * d.plane + o] = vc;
   }
 }
 
@@ -60,7 +64,7 @@ __global__ void gather_kernel(const Dev d, const double* __restrict__ S, double*
     const int sx = wrapi(x - cx(i), nx);
     int sy = y - cy(i);
     if (d.periodic_y) sy = wrapi(sy, ny);
-    const long long o = (long long)(sy + 1) * nx + sx;
+    const long long o = d.at(sx, sy);
     if (a) a[i * n + q] = sol ? 0.0 : S[i * d.plane + o];
     if (b) b[i * n + q] = sol ? 0.0 : S[(9 + i) * d.plane + o];
     if (c) c[i * n + q] = sol ? 0.0 : S[(18 + i) * d.plane + o];
@@ -84,6 +88,21 @@ __global__ void build_links_kernel(const Dev d, int* __restrict__ sites, int* __
 #pragma unroll
   for (int i = 1; i < 9; i++) touches |= fluid_at(d, wrapi(x + cx(i), nx), y + cy(i));
   if (touches) sites[atomicAdd(count, 1)] = (int)q;
+}
+
+// Padded copy of the flag field for the fused kernel: [ny][px], lattice column x at kXL + x, ghost
+// columns = periodic images, everything beyond them solid (never computed on).
+__global__ void pad_mask_kernel(const Dev d, uint8_t* __restrict__ solidp) {
+  const size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= (size_t)d.px * d.ny) return;
+  const int gx = (int)(k % d.px) - kXL, y = (int)(k / d.px);
+  uint8_t v = 1;
+  if (gx >= -kGhost && gx < d.nx + kGhost) {
+    int x = gx % d.nx;
+    if (x < 0) x += d.nx;
+    v = d.solid[(size_t)y * d.nx + x] ? 1 : 0;
+  }
+  solidp[k] = v;
 }
 
 // ---- seeded input recipe (must reproduce paper_2109_12565_b200/inputs.py bit for bit) ----
@@ -206,11 +225,11 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
 }  // namespace
 
 int launch_scatter(const Dev& d, const double* fA, const double* fB, const double* g, double* S, cudaStream_t st) {
-  scatter_kernel<false><<<blocks_for(d.plane, 128), 128, 0, st>>>(d, fA, fB, g, S);
+  scatter_kernel<false><<<blocks_for((long long)(d.nx + 2 * kGhost) * (d.ny + 2), 128), 128, 0, st>>>(d, fA, fB, g, S);
   return 1;
 }
 int launch_set_fields(const Dev& d, const double* rhoA, const double* rhoB, const double* T, double* S, cudaStream_t st) {
-  scatter_kernel<true><<<blocks_for(d.plane, 128), 128, 0, st>>>(d, rhoA, rhoB, T, S);
+  scatter_kernel<true><<<blocks_for((long long)(d.nx + 2 * kGhost) * (d.ny + 2), 128), 128, 0, st>>>(d, rhoA, rhoB, T, S);
   return 1;
 }
 int launch_gather(const Dev& d, const double* S, double* fA, double* fB, double* g, cudaStream_t st) {
@@ -221,10 +240,11 @@ int launch_copy_g(const Dev& d, const double* Ssrc, double* Sdst, cudaStream_t s
   copy_g_kernel<<<blocks_for(9 * d.plane, 256), 256, 0, st>>>(d, Ssrc, Sdst);
   return 1;
 }
-int launch_build_links(const Dev& d, int* sites, int* count, cudaStream_t st) {
+int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st) {
   cudaMemsetAsync(count, 0, sizeof(int), st);
   build_links_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, sites, count);
-  return 1;
+  pad_mask_kernel<<<blocks_for((long long)d.px * d.ny, 256), 256, 0, st>>>(d, solidp);
+  return 2;
 }
 int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* centres, int n_centres, uint8_t* inside,
                 uint8_t* solid, double* rhoA, double* rhoB, double* T, cudaStream_t st) {
