@@ -36,7 +36,6 @@ constexpr int kHX = 4;                  // columns fetched beyond the strip on e
 constexpr int kCopyW = kW + 2 * kHX;    // doubles per plane-row copy
 constexpr int kSlots = 4;               // rows of the 18 fluid planes resident in shared memory
 constexpr int kRingRows = 6;            // rows of rho / psi kept in shared memory
-constexpr int kRingW = kW + 4;          // columns of rho / psi per row (2-cell halo each side)
 constexpr int kXL = 16;                 // padded-row offset of lattice column 0
 constexpr int kGhost = kHX;             // ghost columns kept valid on each side
 

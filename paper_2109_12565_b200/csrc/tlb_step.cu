@@ -15,8 +15,10 @@
 //       populations at (x, y).
 // Streaming (Eq. (1)) is the gather of the next step, so stores are never shifted.  The 9 thermal
 // planes are only needed in (2) and go straight to registers (LDG issued before the row barrier).
-// One __syncthreads and one mbarrier wait per row; the copy of row r+2 is issued as soon as the
-// slot of row r-2 has been read, i.e. a full row of compute ahead of its use.
+// The four warps of a CTA never meet at a CTA-wide barrier: each warp keeps its own rho / psi ring
+// for its 32 columns plus a 2-cell halo (the 4 halo columns are recomputed, not exchanged), waits
+// on the mbarrier of the row it needs, and counts itself out of the slot it has finished with; the
+// last warp out issues the copy of row r+2 into that slot, a full row of compute ahead of its use.
 #include <cstdlib>
 
 #include "tlb_internal.cuh"
@@ -94,12 +96,23 @@ __device__ __forceinline__ int wrap_row(int r, int ny) {
   return r < 0 ? r + ny : r;
 }
 
+constexpr int kWarps = kW / 32;
+constexpr int kWR = 32 + 4;            // ring columns per warp: its 32 columns and a 2-cell halo each side
+
 struct Smem {
-  double f[kSlots][18][kCopyW];        // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
-  double ring[kRingRows][4][kRingW];   // rho_A, rho_B, psi^s_A, psi^s_B (columns x0 - 2 .. x0 + kW + 1)
-  uint8_t flag[kRingRows][kRingW + 4]; // 1 = solid / wall node
-  uint64_t full[kSlots];               // mbarriers: row landed
+  double f[kSlots][18][kCopyW];              // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
+  double ring[kWarps][kRingRows][4][kWR];    // per warp: rho_A, rho_B, psi^s_A, psi^s_B
+  uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
+  uint64_t full[kSlots];                     // mbarriers: row landed
+  unsigned int done[kSlots];                 // warps that have finished reading the slot (running count)
 };
+
+// acq_rel arrive on a shared counter; returns the previous value
+__device__ __forceinline__ unsigned int count_out(unsigned int* c) {
+  unsigned int old;
+  asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(c)) : "memory");
+  return old;
+}
 
 }  // namespace
 
@@ -112,7 +125,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   extern __shared__ __align__(128) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
-  const int t = threadIdx.x;
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const int nx = d.nx, ny = d.ny, px = d.px;
   const int x0 = blockIdx.x * kW;
   const int x = x0 + t;                       // phase-2 column of this thread
@@ -124,7 +137,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
 
   if (t == 0) {
 #pragma unroll
-    for (int s = 0; s < kSlots; s++) mbar_init(&sm.full[s], 1);
+    for (int s = 0; s < kSlots; s++) { mbar_init(&sm.full[s], 1); sm.done[s] = 0; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -156,14 +169,18 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   if (t == 0)
     for (int q = 0; q < 4 && q < q_end; q++) issue(q);
 
-  // phase-1 columns of this thread: c = t (x = x0 - 2 + t) and, for t < 4, c = kW + t
-  const bool extra = t < kRingW - kW;
+  // phase-1 columns of this lane within its warp's ring: c = lane (x = x0 + 32 wid - 2 + lane) and,
+  // for lane < 4, c = 32 + lane
+  const bool extra = lane < kWR - 32;
+  const int xw = x0 + 32 * wid - 2;           // lattice column of ring column 0
   auto mask_at = [&](int r, int c) -> uint8_t {
     if (!row_valid(r)) return 1;
     const int rr = periodic ? wrap_row(r, ny) : r;
-    return d.solidp[(size_t)rr * px + kXL + x0 - 2 + c];
+    return d.solidp[(size_t)rr * px + kXL + xw + c];
   };
-  uint8_t m0 = mask_at(y0 - 2, t), m1 = extra ? mask_at(y0 - 2, kW + t) : 1;
+  uint8_t m0 = mask_at(y0 - 2, lane), m1 = extra ? mask_at(y0 - 2, 32 + lane) : 1;
+  double (*ring)[4][kWR] = sm.ring[wid];
+  uint8_t (*flag)[kWR + 4] = sm.flag[wid];
 
   uint32_t parity = 0;  // one bit per slot
   for (int q = 0; q < q_end; q++) {
@@ -172,16 +189,14 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     const bool valid = row_valid(r);
     const uint8_t s0 = m0, s1 = m1;
     if (q + 1 < q_end) {  // mask of the next row, a full iteration ahead of its use
-      m0 = mask_at(r + 1, t);
-      if (extra) m1 = mask_at(r + 1, kW + t);
+      m0 = mask_at(r + 1, lane);
+      if (extra) m1 = mask_at(r + 1, 32 + lane);
     }
     // thermal populations of row y = r - 2 (phase 2), issued now, consumed after the force stencil
     const int y = r - 2;
     const bool do2 = y >= y0;
     const bool active = do2 && x < nx;
     double g[9];
-#pragma unroll
-    for (int i = 0; i < 9; i++) g[i] = 0.0;
     if (active) {
       int ym = y - 1, yp = y + 1;
       if (periodic) {
@@ -205,23 +220,24 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
 #pragma unroll
     for (int pass = 0; pass < 2; pass++) {
       if (pass == 1 && !extra) break;
-      const int c = pass == 0 ? t : kW + t;
+      const int c = pass == 0 ? lane : 32 + lane;
+      const int cf = 32 * wid + c + 2;  // column of the landed rows holding S(x), x = xw + c
       const uint8_t sol = pass == 0 ? s0 : s1;
       double ra = d.rho_wall_A, rb = d.rho_wall_B, pa = d.pss_wall_A, pb = d.pss_wall_B;
       if (!sol) {
         double fa[9], fb[9];
 #pragma unroll
         for (int i = 0; i < 9; i++) {
-          fa[i] = sm.f[slot][i][c + 2 - cx(i)];
-          fb[i] = sm.f[slot][9 + i][c + 2 - cx(i)];
+          fa[i] = sm.f[slot][i][cf - cx(i)];
+          fb[i] = sm.f[slot][9 + i][cf - cx(i)];
         }
         ra = sum9(fa);
         rb = sum9(fb);
         pa = d.rho0 * (1.0 - exp(-ra * d.inv_rho0));
         pb = d.rho0 * (1.0 - exp(-rb * d.inv_rho0));
       }
-      sm.ring[rq][0][c] = ra; sm.ring[rq][1][c] = rb; sm.ring[rq][2][c] = pa; sm.ring[rq][3][c] = pb;
-      sm.flag[rq][c] = sol;
+      ring[rq][0][c] = ra; ring[rq][1][c] = rb; ring[rq][2][c] = pa; ring[rq][3][c] = pb;
+      flag[rq][c] = sol;
     }
     // the 18 fluid populations of (x, y), landed two iterations ago
     double fa[9], fb[9];
@@ -233,14 +249,15 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         fb[i] = sm.f[slot2][9 + i][t + kHX - cx(i)];
       }
     }
-    __syncthreads();
-    if (t == 0 && q >= 2 && q + 2 < q_end) issue(q + 2);  // slot2 is free: every thread has read it
+    __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
+    if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1 && q + 2 < q_end)
+      issue(q + 2);  // last warp out: the slot is free
     if (!do2) continue;
     // ---- (2) collide row y = r - 2, whose stencil rows y-2..y+2 = r-4..r are resident
     const int rq0 = (q + kRingRows - 2) % kRingRows;  // ring row of y
-    const int cc = t + 2;                             // ring column of x
-    if (active && !sm.flag[rq0][cc]) {
-      const double ra = sm.ring[rq0][0][cc], rb = sm.ring[rq0][1][cc], pa = sm.ring[rq0][2][cc], pb = sm.ring[rq0][3][cc];
+    const int cc = lane + 2;                          // ring column of x
+    if (active && !flag[rq0][cc]) {
+      const double ra = ring[rq0][0][cc], rb = ring[rq0][1][cc], pa = ring[rq0][2][cc], pb = ring[rq0][3][cc];
       // force sums over the 5x5 neighbourhood: cross (w, other species' rho), self (G_a w + G_r p, own psi^s)
       double xAx = 0, xAy = 0, xBx = 0, xBy = 0, sAx = 0, sAy = 0, sBx = 0, sBy = 0;
 #pragma unroll
@@ -251,12 +268,12 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
           const int c2 = dx * dx + dy * dy;
           if (c2 == 0) continue;
           const double w = w_c2(c2), p = p_c2(c2);
-          const double nsA = sm.ring[sl][2][cc + dx], nsB = sm.ring[sl][3][cc + dx];
+          const double nsA = ring[sl][2][cc + dx], nsB = ring[sl][3][cc + dx];
           const double kA = d.G11a * w + d.G11r * p, kB = d.G22a * w + d.G22r * p;
           if (dx != 0) { sAx += (kA * dx) * nsA; sBx += (kB * dx) * nsB; }
           if (dy != 0) { sAy += (kA * dy) * nsA; sBy += (kB * dy) * nsB; }
           if (c2 <= 2) {
-            const double nrA = sm.ring[sl][0][cc + dx], nrB = sm.ring[sl][1][cc + dx];
+            const double nrA = ring[sl][0][cc + dx], nrB = ring[sl][1][cc + dx];
             if (dx != 0) { xAx += (w * dx) * nrB; xBx += (w * dx) * nrA; }
             if (dy != 0) { xAy += (w * dy) * nrB; xBy += (w * dy) * nrA; }
           }
