@@ -40,17 +40,6 @@ __device__ __forceinline__ double sum9(const double (&f)[9]) {  // Eq. (4), same
   return r;
 }
 
-// BGK relaxation towards the second-order equilibrium, Eqs. (2), (3) (c_s^2 = 1/3)
-__device__ __forceinline__ void collide9(double (&f)[9], double dens, double ux, double uy, double omega) {
-  const double usq = 1.0 - 1.5 * (ux * ux + uy * uy);
-#pragma unroll
-  for (int i = 0; i < 9; i++) {
-    const double cu = cx(i) * ux + cy(i) * uy;
-    const double feq = wq(i) * dens * (usq + 3.0 * cu + 4.5 * cu * cu);
-    f[i] = f[i] + omega * (feq - f[i]);
-  }
-}
-
 // ---- mbarrier / bulk-copy primitives (PTX; sm_90+ programming model, sm_100a target) ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -96,12 +85,14 @@ __device__ __forceinline__ int wrap_row(int r, int ny) {
   return r < 0 ? r + ny : r;
 }
 
-constexpr int kWarps = kW / 32;
-constexpr int kWR = 32 + 4;            // ring columns per warp: its 32 columns and a 2-cell halo each side
+constexpr int kThreads = 2 * kW;       // two threads per lattice column: lane 2k = species A, 2k+1 = species B
+constexpr int kWarps = kThreads / 32;  // 8
+constexpr int kWC = 16;                // lattice columns per warp
+constexpr int kWR = kWC + 4;           // ring columns per warp: its 16 columns and a 2-cell halo each side
 
 struct Smem {
   double f[kSlots][18][kCopyW];              // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
-  double ring[kWarps][kRingRows][4][kWR];    // per warp: rho_A, rho_B, psi^s_A, psi^s_B
+  double ring[kWarps][kRingRows][kWR][4];    // per warp: {rho_A, rho_B, psi^s_A, psi^s_B} per column
   uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
   uint64_t full[kSlots];                     // mbarriers: row landed
   unsigned int done[kSlots];                 // warps that have finished reading the slot (running count)
@@ -113,12 +104,24 @@ __device__ __forceinline__ unsigned int count_out(unsigned int* c) {
   asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(c)) : "memory");
   return old;
 }
+__device__ __forceinline__ double pair(double v) { return __shfl_xor_sync(0xffffffffu, v, 1); }  // the other species' lane
+
+// BGK relaxation of one population towards the second-order equilibrium, Eqs. (2), (3) (c_s^2 = 1/3);
+// cu = c_i . u, usq = 1 - 1.5 |u|^2, wd = w_i * density
+__device__ __forceinline__ double relax(double f, double wd, double cu, double usq, double omega) {
+  const double feq = wd * (usq + 3.0 * cu + 4.5 * cu * cu);
+  return f + omega * (feq - f);
+}
 
 }  // namespace
 
 // MODE 0: time step (writes Sout).  MODE 1: hydrodynamic fields of the current state.
-template <int MODE>
-__global__ void __launch_bounds__(kW, 2)
+// Work split inside a lane pair (s = lane & 1): lane s owns species s -- its density and psi^s
+// (phase 1), its force, shifted velocity, collision and 9 stores (phase 2) -- and half of the thermal
+// set: s = 0 takes g_0, g_1, g_2, g_5, g_6, s = 1 the opposite directions g_3, g_4, g_7, g_8, so both
+// lanes run the same code on (c_i, u) and (-c_i, -u).  Partial sums (j, F, T) cross by one shuffle.
+template <int MODE, bool PERIODIC>
+__global__ void __launch_bounds__(kThreads, 2)
 fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ Sout, int seg_rows,
              double* __restrict__ oRA, double* __restrict__ oRB, double* __restrict__ oUx, double* __restrict__ oUy,
              double* __restrict__ oT) {
@@ -126,32 +129,34 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  const int k = lane >> 1, s = lane & 1;
   const int nx = d.nx, ny = d.ny, px = d.px;
   const int x0 = blockIdx.x * kW;
-  const int x = x0 + t;                       // phase-2 column of this thread
+  const int xw = x0 + kWC * wid - 2;          // lattice column of this warp's ring column 0
+  const int x = xw + 2 + k;                   // phase-2 column of this lane pair
   const int y0 = blockIdx.y * seg_rows;
   const int y1 = min(ny, y0 + seg_rows);
   const long long plane = d.plane;
-  const bool periodic = d.periodic_y != 0;
+  const long long planeB = plane * 8, rowB = (long long)px * 8;
   const uint64_t pol = policy_evict_first();  // every line of Sin is dead once read, Sout until the next step
 
   if (t == 0) {
 #pragma unroll
-    for (int s = 0; s < kSlots; s++) { mbar_init(&sm.full[s], 1); sm.done[s] = 0; }
+    for (int i = 0; i < kSlots; i++) { mbar_init(&sm.full[i], 1); sm.done[i] = 0; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
 
   // rows are addressed by q = r - (y0 - 2) >= 0: f slot q & 3, ring row q % 6
   const int q_end = (y1 + 2) - (y0 - 2);      // rows r = y0-2 .. y1+1
-  auto row_valid = [&](int r) { return periodic || (r >= 0 && r < ny); };
-  // elected thread: bring target row r (18 shifted plane rows) into slot q & 3
+  auto row_valid = [&](int r) { return PERIODIC || (r >= 0 && r < ny); };
+  // elected lane: bring target row r (18 shifted plane rows) into slot q & 3
   auto issue = [&](int q) {
     const int r = y0 - 2 + q;
     if (!row_valid(r)) return;
-    const int rr = periodic ? wrap_row(r, ny) : r;
+    const int rr = PERIODIC ? wrap_row(r, ny) : r;
     int rm = rr - 1, rp = rr + 1;             // rows holding the sources of c_y = +1 / -1
-    if (periodic) {
+    if (PERIODIC) {
       if (rm < 0) rm = ny - 1;
       if (rp >= ny) rp = 0;
     }
@@ -159,28 +164,41 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     mbar_expect_tx(bar, 18u * kCopyW * 8u);
     const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
 #pragma unroll
-    for (int s = 0; s < 2; s++)
+    for (int l = 0; l < 2; l++)
 #pragma unroll
       for (int i = 0; i < 9; i++) {
         const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-        bulk_g2s(&sm.f[q & 3][s * 9 + i][0], Sin + (s * 9 + i) * plane + o, kCopyW * 8u, bar, pol);
+        bulk_g2s(&sm.f[q & 3][l * 9 + i][0], Sin + (l * 9 + i) * plane + o, kCopyW * 8u, bar, pol);
       }
   };
   if (t == 0)
     for (int q = 0; q < 4 && q < q_end; q++) issue(q);
 
-  // phase-1 columns of this lane within its warp's ring: c = lane (x = x0 + 32 wid - 2 + lane) and,
-  // for lane < 4, c = 32 + lane
-  const bool extra = lane < kWR - 32;
-  const int xw = x0 + 32 * wid - 2;           // lattice column of ring column 0
+  // phase-1 tasks of this lane: ring column k and, for lanes < 8, ring column 16 + k; species s
+  const bool extra = lane < 2 * (kWR - kWC);
   auto mask_at = [&](int r, int c) -> uint8_t {
     if (!row_valid(r)) return 1;
-    const int rr = periodic ? wrap_row(r, ny) : r;
+    const int rr = PERIODIC ? wrap_row(r, ny) : r;
     return d.solidp[(size_t)rr * px + kXL + xw + c];
   };
-  uint8_t m0 = mask_at(y0 - 2, lane), m1 = extra ? mask_at(y0 - 2, 32 + lane) : 1;
-  double (*ring)[4][kWR] = sm.ring[wid];
+  uint8_t m0 = mask_at(y0 - 2, k), m1 = extra ? mask_at(y0 - 2, kWC + k) : 1;
+  double (*ring)[kWR][4] = sm.ring[wid];
   uint8_t (*flag)[kWR + 4] = sm.flag[wid];
+
+  // per-lane constants: own wall values, own self-interaction stencil coefficients G^a w + G^r p by |c|^2
+  const double rho_wall = s ? d.rho_wall_B : d.rho_wall_A, pss_wall = s ? d.pss_wall_B : d.pss_wall_A;
+  const double Ga = s ? d.G22a : d.G11a, Gr = s ? d.G22r : d.G11r;
+  const double k1 = Ga * w_c2(1) + Gr * p_c2(1), k2 = Ga * w_c2(2) + Gr * p_c2(2), k4 = Ga * w_c2(4) + Gr * p_c2(4),
+               k5 = Ga * w_c2(5) + Gr * p_c2(5), k8 = Ga * w_c2(8) + Gr * p_c2(8);
+  const double k4d = 2.0 * k4, k5d = 2.0 * k5, k8d = 2.0 * k8;
+  const double gx = d.G12 * d.inv_rho0 * d.inv_rho0;  // Eqs. (7), (8): psi^x = rho / rho0 on both factors
+  const double sgn = s ? -1.0 : 1.0;                  // this lane's thermal directions are sgn * {c_1, c_2, c_5, c_6}
+
+  // running byte pointers of row y = y0 (advanced by one row per phase-2 iteration)
+  const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + d.at(x, y0));   // g_{i + 2s}
+  char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + d.at(x, y0));                    // own species
+  char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + d.at(x, y0));             // own thermal half
+  const int co = s ? 8 : -8;                                                                    // x - c_x of c_1 / c_3
 
   uint32_t parity = 0;  // one bit per slot
   for (int q = 0; q < q_end; q++) {
@@ -189,30 +207,27 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     const bool valid = row_valid(r);
     const uint8_t s0 = m0, s1 = m1;
     if (q + 1 < q_end) {  // mask of the next row, a full iteration ahead of its use
-      m0 = mask_at(r + 1, lane);
-      if (extra) m1 = mask_at(r + 1, 32 + lane);
+      m0 = mask_at(r + 1, k);
+      if (extra) m1 = mask_at(r + 1, kWC + k);
     }
-    // thermal populations of row y = r - 2 (phase 2), issued now, consumed after the force stencil
-    const int y = r - 2;
+    const int y = r - 2;        // row of phase 2
     const bool do2 = y >= y0;
-    const bool active = do2 && x < nx;
-    double g[9];
-    if (active) {
-      int ym = y - 1, yp = y + 1;
-      if (periodic) {
-        if (ym < 0) ym = ny - 1;
-        if (yp >= ny) yp = 0;
+    // thermal populations of (x, y): issued now, consumed after the force stencil.  Lane s = 0 reads
+    // g_0, g_1, g_2, g_5, g_6 at x - c_i; lane s = 1 the opposite directions at x + c_i.
+    double g0 = 0.0, ga = 0.0, gb = 0.0, gc = 0.0, gd = 0.0;
+    if (do2) {
+      long long rofs = s ? rowB : -rowB;  // row y - c_y of this lane's c_y = +-1 directions
+      if (PERIODIC) {
+        if (!s && y == 0) rofs = (long long)(ny - 1) * rowB;
+        if (s && y == ny - 1) rofs = -(long long)(ny - 1) * rowB;
       }
-      const double* g0 = Sin + 18 * plane + d.at(x, y);
-      const double* gm = Sin + 18 * plane + d.at(x, ym);
-      const double* gp = Sin + 18 * plane + d.at(x, yp);
-#pragma unroll
-      for (int i = 0; i < 9; i++) {
-        const double* b = cy(i) == 0 ? g0 : (cy(i) > 0 ? gm : gp);
-        g[i] = ldg_stream(b + i * plane - cx(i), pol);
-      }
+      g0 = ldg_stream(reinterpret_cast<const double*>(gp - (s ? 2 * planeB : 0)), pol);
+      ga = ldg_stream(reinterpret_cast<const double*>(gp + 1 * planeB + co), pol);
+      gb = ldg_stream(reinterpret_cast<const double*>(gp + 2 * planeB + rofs), pol);
+      gc = ldg_stream(reinterpret_cast<const double*>(gp + 5 * planeB + rofs + co), pol);
+      gd = ldg_stream(reinterpret_cast<const double*>(gp + 6 * planeB + rofs - co), pol);
     }
-    // ---- (1) rho, psi of row r (Eqs. (4), (12)); wall values at solid / out-of-domain nodes (L155, R9)
+    // ---- (1) rho_s, psi^s_s of row r (Eqs. (4), (12)); wall values at solid / out-of-domain nodes (L155, R9)
     if (valid) {
       mbar_wait(&sm.full[slot], (parity >> slot) & 1u);
       parity ^= 1u << slot;
@@ -220,116 +235,150 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
 #pragma unroll
     for (int pass = 0; pass < 2; pass++) {
       if (pass == 1 && !extra) break;
-      const int c = pass == 0 ? lane : 32 + lane;
-      const int cf = 32 * wid + c + 2;  // column of the landed rows holding S(x), x = xw + c
+      const int c = pass == 0 ? k : kWC + k;
       const uint8_t sol = pass == 0 ? s0 : s1;
-      double ra = d.rho_wall_A, rb = d.rho_wall_B, pa = d.pss_wall_A, pb = d.pss_wall_B;
+      double rl = rho_wall, pl = pss_wall;
       if (!sol) {
-        double fa[9], fb[9];
+        const double* fs = &sm.f[slot][9 * s][kWC * wid + c + 2];  // S(x) of ring column c
+        double f[9];
 #pragma unroll
-        for (int i = 0; i < 9; i++) {
-          fa[i] = sm.f[slot][i][cf - cx(i)];
-          fb[i] = sm.f[slot][9 + i][cf - cx(i)];
-        }
-        ra = sum9(fa);
-        rb = sum9(fb);
-        pa = d.rho0 * (1.0 - exp(-ra * d.inv_rho0));
-        pb = d.rho0 * (1.0 - exp(-rb * d.inv_rho0));
+        for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
+        rl = sum9(f);
+        pl = d.rho0 * (1.0 - exp(-rl * d.inv_rho0));
       }
-      ring[rq][0][c] = ra; ring[rq][1][c] = rb; ring[rq][2][c] = pa; ring[rq][3][c] = pb;
+      ring[rq][c][s] = rl;
+      ring[rq][c][2 + s] = pl;
       flag[rq][c] = sol;
     }
-    // the 18 fluid populations of (x, y), landed two iterations ago
-    double fa[9], fb[9];
+    // the 9 own-species populations of (x, y), landed two iterations ago
     const int slot2 = (q + 2) & 3;  // == (q - 2) & 3
-    if (active) {
+    double f[9];
+    {
+      const double* fs = &sm.f[slot2][9 * s][kWC * wid + k + kHX];
 #pragma unroll
-      for (int i = 0; i < 9; i++) {
-        fa[i] = sm.f[slot2][i][t + kHX - cx(i)];
-        fb[i] = sm.f[slot2][9 + i][t + kHX - cx(i)];
-      }
+      for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
     }
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
     if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1 && q + 2 < q_end)
       issue(q + 2);  // last warp out: the slot is free
     if (!do2) continue;
+
     // ---- (2) collide row y = r - 2, whose stencil rows y-2..y+2 = r-4..r are resident
     const int rq0 = (q + kRingRows - 2) % kRingRows;  // ring row of y
-    const int cc = lane + 2;                          // ring column of x
-    if (active && !flag[rq0][cc]) {
-      const double ra = ring[rq0][0][cc], rb = ring[rq0][1][cc], pa = ring[rq0][2][cc], pb = ring[rq0][3][cc];
-      // force sums over the 5x5 neighbourhood: cross (w, other species' rho), self (G_a w + G_r p, own psi^s)
-      double xAx = 0, xAy = 0, xBx = 0, xBy = 0, sAx = 0, sAy = 0, sBx = 0, sBy = 0;
+    const int cc = k + 2;                             // ring column of x
+    const bool fluid = x < nx && !flag[rq0][cc];
+    const double rl = ring[rq0][cc][s], rn = ring[rq0][cc][1 - s], pl = ring[rq0][cc][2 + s];
+    // force sums over the 5x5 neighbourhood: cross (w, other species' rho), self (G_a w + G_r p, own psi^s)
+    double Xx = 0, Xy = 0, Sx = 0, Sy = 0;
 #pragma unroll
-      for (int dy = -2; dy <= 2; dy++) {
-        const int sl = (q + kRingRows - 2 + dy) % kRingRows;
+    for (int dy = -2; dy <= 2; dy++) {
+      const int sl = (q + kRingRows - 2 + dy) % kRingRows;
 #pragma unroll
-        for (int dx = -2; dx <= 2; dx++) {
-          const int c2 = dx * dx + dy * dy;
-          if (c2 == 0) continue;
-          const double w = w_c2(c2), p = p_c2(c2);
-          const double nsA = ring[sl][2][cc + dx], nsB = ring[sl][3][cc + dx];
-          const double kA = d.G11a * w + d.G11r * p, kB = d.G22a * w + d.G22r * p;
-          if (dx != 0) { sAx += (kA * dx) * nsA; sBx += (kB * dx) * nsB; }
-          if (dy != 0) { sAy += (kA * dy) * nsA; sBy += (kB * dy) * nsB; }
-          if (c2 <= 2) {
-            const double nrA = ring[sl][0][cc + dx], nrB = ring[sl][1][cc + dx];
-            if (dx != 0) { xAx += (w * dx) * nrB; xBx += (w * dx) * nrA; }
-            if (dy != 0) { xAy += (w * dy) * nrB; xBy += (w * dy) * nrA; }
-          }
+      for (int dx = -2; dx <= 2; dx++) {
+        const int c2 = dx * dx + dy * dy;
+        if (c2 == 0) continue;
+        const double kk = c2 == 1 ? k1 : c2 == 2 ? k2 : c2 == 4 ? k4 : c2 == 5 ? k5 : k8;      // |component| = 1
+        const double kd = c2 == 4 ? k4d : c2 == 5 ? k5d : k8d;                                  // |component| = 2
+        const double ns = ring[sl][cc + dx][2 + s];
+        if (dx > 0) Sx += (dx == 1 ? kk : kd) * ns;
+        if (dx < 0) Sx -= (dx == -1 ? kk : kd) * ns;
+        if (dy > 0) Sy += (dy == 1 ? kk : kd) * ns;
+        if (dy < 0) Sy -= (dy == -1 ? kk : kd) * ns;
+        if (c2 <= 2) {
+          const double nr = ring[sl][cc + dx][1 - s];
+          if (dx != 0) Xx += (w_c2(c2) * dx) * nr;
+          if (dy != 0) Xy += (w_c2(c2) * dy) * nr;
         }
       }
-      // Eqs. (7), (8): psi^x = rho / rho0 on both factors
-      const double gx = d.G12 * d.inv_rho0 * d.inv_rho0;
-      double FAx = -gx * ra * xAx - pa * sAx, FAy = -gx * ra * xAy - pa * sAy;
-      double FBx = -gx * rb * xBx - pb * sBx, FBy = -gx * rb * xBy - pb * sBy;
-      // moments, Eqs. (5), (17)
-      const double T = sum9(g);
-      const double jx = (fa[1] - fa[3] + fa[5] - fa[6] - fa[7] + fa[8]) + (fb[1] - fb[3] + fb[5] - fb[6] - fb[7] + fb[8]);
-      const double jy = (fa[2] - fa[4] + fa[5] + fa[6] - fa[7] - fa[8]) + (fb[2] - fb[4] + fb[5] + fb[6] - fb[7] - fb[8]);
-      // Eq. (22) buoyancy (R12) and the x-acceleration extension
-      const double dT = d.thermal ? (T - d.T_ref) : 0.0;
-      FAy += ra * d.alpha_g * dT; FBy += rb * d.alpha_g * dT;
-      FAx += ra * d.body_ax;      FBx += rb * d.body_ax;
-      const double rho = ra + rb;
-      const double inv = 1.0 / rho, invA = d.tau / ra, invB = d.tau / rb;
-      const double ux = jx * inv, uy = jy * inv;                       // Eq. (5)
-      const double uHx = (jx + 0.5 * (FAx + FBx)) * inv, uHy = (jy + 0.5 * (FAy + FBy)) * inv;  // L139
-      if (MODE == 1) {
-        const size_t k = (size_t)y * nx + x;
-        if (oRA) oRA[k] = ra;
-        if (oRB) oRB[k] = rb;
-        if (oUx) oUx[k] = uHx;
-        if (oUy) oUy[k] = uHy;
-        if (oT) oT[k] = T;
-      } else {
-        collide9(fa, ra, ux + FAx * invA, uy + FAy * invA, d.omega);  // Eq. (6)
-        collide9(fb, rb, ux + FBx * invB, uy + FBy * invB, d.omega);
-        if (d.thermal) collide9(g, T, uHx, uHy, d.omega_g);           // Eqs. (16), (18)
-        double* o = Sout + d.at(x, y);
-        const int nsets = d.thermal ? 27 : 18;
-#pragma unroll
-        for (int i = 0; i < 27; i++)
-          if (i < nsets) stg_stream(o + i * plane, i < 9 ? fa[i] : (i < 18 ? fb[i - 9] : g[i - 18]), pol);
-        if (x < kGhost || x >= nx - kGhost) {  // periodic images of this column (ghost columns)
-          for (int xg = x + nx; xg < nx + kGhost; xg += nx)
-#pragma unroll
-            for (int i = 0; i < 27; i++)
-              if (i < nsets) o[i * plane + (xg - x)] = i < 9 ? fa[i] : (i < 18 ? fb[i - 9] : g[i - 18]);
-          for (int xg = x - nx; xg >= -kGhost; xg -= nx)
-#pragma unroll
-            for (int i = 0; i < 27; i++)
-              if (i < nsets) o[i * plane + (xg - x)] = i < 9 ? fa[i] : (i < 18 ? fb[i - 9] : g[i - 18]);
-        }
-      }
-    } else if (MODE == 1 && active) {  // solid site: report the wall values
-      const size_t k = (size_t)y * nx + x;
-      if (oRA) oRA[k] = d.rho_wall_A;
-      if (oRB) oRB[k] = d.rho_wall_B;
-      if (oUx) oUx[k] = 0.0;
-      if (oUy) oUy[k] = 0.0;
-      if (oT) oT[k] = (2 * y < ny) ? d.T_bottom : d.T_top;
     }
+    double Fx = -gx * rl * Xx - pl * Sx, Fy = -gx * rl * Xy - pl * Sy;
+    // moments, Eqs. (5), (17): partial sums of this lane + the other species' lane
+    const double Tp = (s ? 0.0 : g0) + ga + gb + gc + gd;
+    const double T = Tp + pair(Tp);
+    const double jxl = f[1] - f[3] + f[5] - f[6] - f[7] + f[8];
+    const double jyl = f[2] - f[4] + f[5] + f[6] - f[7] - f[8];
+    const double jx = jxl + pair(jxl), jy = jyl + pair(jyl);
+    // Eq. (22) buoyancy (R12) and the x-acceleration extension
+    const double dT = d.thermal ? (T - d.T_ref) : 0.0;
+    Fy += rl * d.alpha_g * dT;
+    Fx += rl * d.body_ax;
+    const double rho = rl + rn;
+    const double inv = 1.0 / rho, invl = d.tau / rl;
+    const double ux = jx * inv, uy = jy * inv;                      // Eq. (5)
+    const double Ftx = Fx + pair(Fx), Fty = Fy + pair(Fy);
+    const double uHx = (jx + 0.5 * Ftx) * inv, uHy = (jy + 0.5 * Fty) * inv;  // L139
+    if (MODE == 1) {
+      if (x < nx) {
+        const size_t o = (size_t)y * nx + x;
+        double* o1 = s ? oRB : oRA;
+        double* o2 = s ? oUy : oUx;
+        if (fluid) {
+          if (o1) o1[o] = rl;
+          if (o2) o2[o] = s ? uHy : uHx;
+          if (!s && oT) oT[o] = T;
+        } else {  // solid site: report the wall values
+          if (o1) o1[o] = rho_wall;
+          if (o2) o2[o] = 0.0;
+          if (!s && oT) oT[o] = (2 * y < ny) ? d.T_bottom : d.T_top;
+        }
+      }
+    } else {
+      // own species: Eq. (6) shifted velocity, Eqs. (2), (3)
+      {
+        const double vx = ux + Fx * invl, vy = uy + Fy * invl;
+        const double usq = 1.0 - 1.5 * (vx * vx + vy * vy);
+        const double w0 = wq(0) * rl, w1 = wq(1) * rl, w5 = wq(5) * rl;
+        f[0] = relax(f[0], w0, 0.0, usq, d.omega);
+        f[1] = relax(f[1], w1, vx, usq, d.omega);
+        f[2] = relax(f[2], w1, vy, usq, d.omega);
+        f[3] = relax(f[3], w1, -vx, usq, d.omega);
+        f[4] = relax(f[4], w1, -vy, usq, d.omega);
+        f[5] = relax(f[5], w5, vx + vy, usq, d.omega);
+        f[6] = relax(f[6], w5, -vx + vy, usq, d.omega);
+        f[7] = relax(f[7], w5, -vx - vy, usq, d.omega);
+        f[8] = relax(f[8], w5, vx - vy, usq, d.omega);
+      }
+      // own half of the thermal set: Eqs. (16), (18) with u^(H); directions sgn * {c_1, c_2, c_5, c_6}
+      if (d.thermal) {
+        const double vx = sgn * uHx, vy = sgn * uHy;
+        const double usq = 1.0 - 1.5 * (uHx * uHx + uHy * uHy);
+        const double w0 = wq(0) * T, w1 = wq(1) * T, w5 = wq(5) * T;
+        g0 = relax(g0, w0, 0.0, usq, d.omega_g);
+        ga = relax(ga, w1, vx, usq, d.omega_g);
+        gb = relax(gb, w1, vy, usq, d.omega_g);
+        gc = relax(gc, w5, vx + vy, usq, d.omega_g);
+        gd = relax(gd, w5, -vx + vy, usq, d.omega_g);
+      }
+      if (fluid) {
+#pragma unroll
+        for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<double*>(opf + i * planeB), f[i], pol);
+        if (d.thermal) {
+          if (!s) stg_stream(reinterpret_cast<double*>(opg), g0, pol);
+          stg_stream(reinterpret_cast<double*>(opg + 1 * planeB), ga, pol);
+          stg_stream(reinterpret_cast<double*>(opg + 2 * planeB), gb, pol);
+          stg_stream(reinterpret_cast<double*>(opg + 5 * planeB), gc, pol);
+          stg_stream(reinterpret_cast<double*>(opg + 6 * planeB), gd, pol);
+        }
+        if (x < kGhost || x >= nx - kGhost) {  // periodic images of this column (ghost columns)
+          for (int pass = 0; pass < 2; pass++)
+            for (int xg = pass ? x - nx : x + nx; pass ? xg >= -kGhost : xg < nx + kGhost; xg += pass ? -nx : nx) {
+              const long long e = (long long)(xg - x) * 8;
+#pragma unroll
+              for (int i = 0; i < 9; i++) *reinterpret_cast<double*>(opf + i * planeB + e) = f[i];
+              if (d.thermal) {
+                if (!s) *reinterpret_cast<double*>(opg + e) = g0;
+                *reinterpret_cast<double*>(opg + 1 * planeB + e) = ga;
+                *reinterpret_cast<double*>(opg + 2 * planeB + e) = gb;
+                *reinterpret_cast<double*>(opg + 5 * planeB + e) = gc;
+                *reinterpret_cast<double*>(opg + 6 * planeB + e) = gd;
+              }
+            }
+        }
+      }
+    }
+    gp += rowB;
+    opf += rowB;
+    opg += rowB;
   }
 }
 
@@ -384,9 +433,11 @@ static dim3 strip_grid(const Dev& d, int seg_rows) {
 }
 
 int configure_kernels() {
-  cudaError_t e = cudaFuncSetAttribute(fused_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
-  if (e == cudaSuccess)
-    e = cudaFuncSetAttribute(fused_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(Smem));
+  const int bytes = (int)sizeof(Smem);
+  cudaError_t e = cudaFuncSetAttribute(fused_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
   return e == cudaSuccess ? 0 : (int)e;
 }
 
@@ -412,15 +463,22 @@ int default_seg_rows(int nx, int ny) {
 }
 
 int launch_step(const Dev& d, const double* Sin, double* Sout, int seg_rows, cudaStream_t st) {
-  fused_kernel<0><<<strip_grid(d, seg_rows), kW, sizeof(Smem), st>>>(d, Sin, Sout, seg_rows, nullptr, nullptr, nullptr,
-                                                                     nullptr, nullptr);
+  if (d.periodic_y)
+    fused_kernel<0, true><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, Sin, Sout, seg_rows, nullptr, nullptr,
+                                                                                 nullptr, nullptr, nullptr);
+  else
+    fused_kernel<0, false><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, Sin, Sout, seg_rows, nullptr, nullptr,
+                                                                                  nullptr, nullptr, nullptr);
   return 1;
 }
 
 int launch_fields(const Dev& d, const double* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
                   cudaStream_t st) {
   const int seg_rows = default_seg_rows(d.nx, d.ny);
-  fused_kernel<1><<<strip_grid(d, seg_rows), kW, sizeof(Smem), st>>>(d, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T);
+  if (d.periodic_y)
+    fused_kernel<1, true><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T);
+  else
+    fused_kernel<1, false><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T);
   return 1;
 }
 
