@@ -115,9 +115,11 @@ int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g);
  * one wall/obstacle boundary kernel. */
 int tlb_step(tlb_handle* h, int64_t n);
 
-/* Measurement aid: advance n (1..4096) steps like tlb_step, with CUDA events recorded on the handle's
- * stream around every launch; returns the average duration in milliseconds of the fused kernel and
- * of the boundary kernel (HOST pointers).  Synchronises the stream. */
+/* Measurement aid: advance ONE step, launching the fused kernel n (1..4096) times back to back on the
+ * same input / output buffers and then the boundary kernel n times (both are idempotent on fixed inputs),
+ * with CUDA events recorded on the handle's stream around each batch; returns the average duration in
+ * milliseconds of one fused-kernel launch and of one boundary-kernel launch (HOST pointers).
+ * Synchronises the stream. */
 int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundary_ms);
 
 /* Hydrodynamic fields at the current time: rho_A, rho_B [ny][nx], u = u^(H) [2][ny][nx] (L139),

@@ -57,7 +57,8 @@ def build(force=False, verbose=False):
         return LIB_PATH
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB_PATH + ".%d.tmp" % os.getpid()
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", _INCLUDE, "-o", tmp] + \
+    extra = os.environ.get("TLB_NVCC_EXTRA", "").split()  # experiments only (e.g. -DTLB_EXP=1)
+    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", _INCLUDE, "-o", tmp] + \
           [os.path.join(_CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB_PATH)
@@ -228,7 +229,8 @@ class TLB:
         self._chk(self.lib.tlb_step(self.h, int(n)))
 
     def profile_step(self, n):
-        """(fused_ms, boundary_ms): average kernel durations over n steps, CUDA events on the stream."""
+        """(fused_ms, boundary_ms): average duration of n back-to-back launches of each kernel (CUDA events on the
+        stream); the state advances by one step."""
         a, b = ctypes.c_double(), ctypes.c_double()
         self._chk(self.lib.tlb_profile_step(self.h, int(n), ctypes.byref(a), ctypes.byref(b)))
         return a.value, b.value

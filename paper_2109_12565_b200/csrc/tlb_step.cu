@@ -71,6 +71,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
+// L2 prefetch of `bytes` (multiple of 16, 16-byte aligned): starts the HBM read rows ahead of the copy
+// that needs shared memory, so the depth of the read queue is not bounded by the shared-memory ring
+__device__ __forceinline__ void prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ double ldg_stream(const double* a, uint64_t policy) {
   double v;
   asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(policy));
@@ -85,6 +90,10 @@ __device__ __forceinline__ int wrap_row(int r, int ny) {
   return r < 0 ? r + ny : r;
 }
 
+#ifndef TLB_PREF_D
+#define TLB_PREF_D 4
+#endif
+constexpr int kPrefetchRows = TLB_PREF_D;  // rows the HBM -> L2 prefetch runs ahead of the shared-memory copy
 constexpr int kThreads = 2 * kW;       // two threads per lattice column: lane 2k = species A, 2k+1 = species B
 constexpr int kWarps = kThreads / 32;  // 8
 constexpr int kWC = 16;                // lattice columns per warp
@@ -92,7 +101,8 @@ constexpr int kWR = kWC + 4;           // ring columns per warp: its 16 columns 
 
 struct Smem {
   double f[kSlots][18][kCopyW];              // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
-  double ring[kWarps][kRingRows][kWR][4];    // per warp: {rho_A, rho_B, psi^s_A, psi^s_B} per column
+  double rho[kWarps][kRingRows][kWR][2];     // per warp: {rho_A, rho_B} per column (a lane pair reads 16 contiguous bytes,
+  double psi[kWarps][kRingRows][kWR][2];     //           {psi^s_A, psi^s_B}          a half-warp 128: conflict-free)
   uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
   uint64_t full[kSlots];                     // mbarriers: row landed
   unsigned int done[kSlots];                 // warps that have finished reading the slot (running count)
@@ -136,8 +146,16 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   const int x = xw + 2 + k;                   // phase-2 column of this lane pair
   const int y0 = blockIdx.y * seg_rows;
   const int y1 = min(ny, y0 + seg_rows);
+#if defined(TLB_EXP) && (TLB_EXP & 2)
+  const int strips_ = gridDim.x;          // EXPERIMENT: (row, strip)-tiled layout, timing only
+  const long long plane = 128;
+  const long long planeB = plane * 8, rowB = (long long)strips_ * 27 * 128 * 8;
+  auto AT = [&](int xx, int yy) { return ((long long)(yy + 1) * strips_ + blockIdx.x) * 27 * 128 + (xx - x0); };
+#else
   const long long plane = d.plane;
   const long long planeB = plane * 8, rowB = (long long)px * 8;
+  auto AT = [&](int xx, int yy) { return d.at(xx, yy); };
+#endif
   const uint64_t pol = policy_evict_first();  // every line of Sin is dead once read, Sout until the next step
 
   if (t == 0) {
@@ -162,7 +180,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     }
     uint64_t* bar = &sm.full[q & 3];
     mbar_expect_tx(bar, 18u * kCopyW * 8u);
-    const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
+    const long long o0 = AT(x0 - kHX, rr), om = AT(x0 - kHX, rm), op = AT(x0 - kHX, rp);
 #pragma unroll
     for (int l = 0; l < 2; l++)
 #pragma unroll
@@ -171,8 +189,29 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         bulk_g2s(&sm.f[q & 3][l * 9 + i][0], Sin + (l * 9 + i) * plane + o, kCopyW * 8u, bar, pol);
       }
   };
-  if (t == 0)
+  // elected lane: start the HBM -> L2 read of all 27 source plane rows of target row r
+  auto prefetch = [&](int q) {
+    const int r = y0 - 2 + q;
+    if (!row_valid(r)) return;
+    const int rr = PERIODIC ? wrap_row(r, ny) : r;
+    int rm = rr - 1, rp = rr + 1;
+    if (PERIODIC) {
+      if (rm < 0) rm = ny - 1;
+      if (rp >= ny) rp = 0;
+    }
+    const long long o0 = AT(x0 - kHX, rr), om = AT(x0 - kHX, rm), op = AT(x0 - kHX, rp);
+    const int np = (d.thermal && q >= 2 && q < q_end - 2) ? 27 : 18;  // g only for rows that reach phase 2
+#pragma unroll
+    for (int p = 0; p < 27; p++) {
+      const int i = p % 9;
+      const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
+      if (p < np) prefetch_l2(Sin + p * plane + o, kCopyW * 8u);
+    }
+  };
+  if (t == 0) {
     for (int q = 0; q < 4 && q < q_end; q++) issue(q);
+    for (int q = 4; q < 4 + kPrefetchRows && q < q_end; q++) prefetch(q);
+  }
 
   // phase-1 tasks of this lane: ring column k and, for lanes < 8, ring column 16 + k; species s
   const bool extra = lane < 2 * (kWR - kWC);
@@ -182,7 +221,8 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     return d.solidp[(size_t)rr * px + kXL + xw + c];
   };
   uint8_t m0 = mask_at(y0 - 2, k), m1 = extra ? mask_at(y0 - 2, kWC + k) : 1;
-  double (*ring)[kWR][4] = sm.ring[wid];
+  double (*rho_r)[kWR][2] = sm.rho[wid];
+  double (*psi_r)[kWR][2] = sm.psi[wid];
   uint8_t (*flag)[kWR + 4] = sm.flag[wid];
 
   // per-lane constants: own wall values, own self-interaction stencil coefficients G^a w + G^r p by |c|^2
@@ -195,10 +235,26 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   const double sgn = s ? -1.0 : 1.0;                  // this lane's thermal directions are sgn * {c_1, c_2, c_5, c_6}
 
   // running byte pointers of row y = y0 (advanced by one row per phase-2 iteration)
-  const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + d.at(x, y0));   // g_{i + 2s}
-  char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + d.at(x, y0));                    // own species
-  char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + d.at(x, y0));             // own thermal half
+  const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + AT(x, y0));   // g_{i + 2s}
+  char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + AT(x, y0));                    // own species
+  char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + AT(x, y0));             // own thermal half
   const int co = s ? 8 : -8;                                                                    // x - c_x of c_1 / c_3
+
+  // thermal populations of (x, y).  Lane s = 0 reads
+  // g_0, g_1, g_2, g_5, g_6 at x - c_i; lane s = 1 the opposite directions at x + c_i.
+  double g0, ga, gb, gc, gd;
+  auto load_g = [&](int y) {
+    long long rofs = s ? rowB : -rowB;  // row y - c_y of this lane's c_y = +-1 directions
+    if (PERIODIC) {
+      if (!s && y == 0) rofs = (long long)(ny - 1) * rowB;
+      if (s && y == ny - 1) rofs = -(long long)(ny - 1) * rowB;
+    }
+    g0 = ldg_stream(reinterpret_cast<const double*>(gp - (s ? 2 * planeB : 0)), pol);
+    ga = ldg_stream(reinterpret_cast<const double*>(gp + 1 * planeB + co), pol);
+    gb = ldg_stream(reinterpret_cast<const double*>(gp + 2 * planeB + rofs), pol);
+    gc = ldg_stream(reinterpret_cast<const double*>(gp + 5 * planeB + rofs + co), pol);
+    gd = ldg_stream(reinterpret_cast<const double*>(gp + 6 * planeB + rofs - co), pol);
+  };
 
   uint32_t parity = 0;  // one bit per slot
   for (int q = 0; q < q_end; q++) {
@@ -212,21 +268,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     }
     const int y = r - 2;        // row of phase 2
     const bool do2 = y >= y0;
-    // thermal populations of (x, y): issued now, consumed after the force stencil.  Lane s = 0 reads
-    // g_0, g_1, g_2, g_5, g_6 at x - c_i; lane s = 1 the opposite directions at x + c_i.
-    double g0 = 0.0, ga = 0.0, gb = 0.0, gc = 0.0, gd = 0.0;
-    if (do2) {
-      long long rofs = s ? rowB : -rowB;  // row y - c_y of this lane's c_y = +-1 directions
-      if (PERIODIC) {
-        if (!s && y == 0) rofs = (long long)(ny - 1) * rowB;
-        if (s && y == ny - 1) rofs = -(long long)(ny - 1) * rowB;
-      }
-      g0 = ldg_stream(reinterpret_cast<const double*>(gp - (s ? 2 * planeB : 0)), pol);
-      ga = ldg_stream(reinterpret_cast<const double*>(gp + 1 * planeB + co), pol);
-      gb = ldg_stream(reinterpret_cast<const double*>(gp + 2 * planeB + rofs), pol);
-      gc = ldg_stream(reinterpret_cast<const double*>(gp + 5 * planeB + rofs + co), pol);
-      gd = ldg_stream(reinterpret_cast<const double*>(gp + 6 * planeB + rofs - co), pol);
-    }
+    if (do2) load_g(y);  // consumed after the force stencil (issuing it a row earlier measured slower)
     // ---- (1) rho_s, psi^s_s of row r (Eqs. (4), (12)); wall values at solid / out-of-domain nodes (L155, R9)
     if (valid) {
       mbar_wait(&sm.full[slot], (parity >> slot) & 1u);
@@ -243,11 +285,15 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         double f[9];
 #pragma unroll
         for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
+#if defined(TLB_EXP) && (TLB_EXP & 4)
+        rl = f[0] + f[8]; pl = rl;
+#else
         rl = sum9(f);
         pl = d.rho0 * (1.0 - exp(-rl * d.inv_rho0));
+#endif
       }
-      ring[rq][c][s] = rl;
-      ring[rq][c][2 + s] = pl;
+      rho_r[rq][c][s] = rl;
+      psi_r[rq][c][s] = pl;
       flag[rq][c] = sol;
     }
     // the 9 own-species populations of (x, y), landed two iterations ago
@@ -259,17 +305,20 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
     }
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
-    if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1 && q + 2 < q_end)
-      issue(q + 2);  // last warp out: the slot is free
+    if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1) {  // last warp out: the slot is free
+      if (q + 2 < q_end) issue(q + 2);
+      if (q + 2 + kPrefetchRows < q_end) prefetch(q + 2 + kPrefetchRows);
+    }
     if (!do2) continue;
 
     // ---- (2) collide row y = r - 2, whose stencil rows y-2..y+2 = r-4..r are resident
     const int rq0 = (q + kRingRows - 2) % kRingRows;  // ring row of y
     const int cc = k + 2;                             // ring column of x
     const bool fluid = x < nx && !flag[rq0][cc];
-    const double rl = ring[rq0][cc][s], rn = ring[rq0][cc][1 - s], pl = ring[rq0][cc][2 + s];
+    const double rl = rho_r[rq0][cc][s], rn = rho_r[rq0][cc][1 - s], pl = psi_r[rq0][cc][s];
     // force sums over the 5x5 neighbourhood: cross (w, other species' rho), self (G_a w + G_r p, own psi^s)
     double Xx = 0, Xy = 0, Sx = 0, Sy = 0;
+#if !defined(TLB_EXP) || !(TLB_EXP & 1)
 #pragma unroll
     for (int dy = -2; dy <= 2; dy++) {
       const int sl = (q + kRingRows - 2 + dy) % kRingRows;
@@ -279,18 +328,19 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         if (c2 == 0) continue;
         const double kk = c2 == 1 ? k1 : c2 == 2 ? k2 : c2 == 4 ? k4 : c2 == 5 ? k5 : k8;      // |component| = 1
         const double kd = c2 == 4 ? k4d : c2 == 5 ? k5d : k8d;                                  // |component| = 2
-        const double ns = ring[sl][cc + dx][2 + s];
+        const double ns = psi_r[sl][cc + dx][s];
         if (dx > 0) Sx += (dx == 1 ? kk : kd) * ns;
         if (dx < 0) Sx -= (dx == -1 ? kk : kd) * ns;
         if (dy > 0) Sy += (dy == 1 ? kk : kd) * ns;
         if (dy < 0) Sy -= (dy == -1 ? kk : kd) * ns;
         if (c2 <= 2) {
-          const double nr = ring[sl][cc + dx][1 - s];
+          const double nr = rho_r[sl][cc + dx][1 - s];
           if (dx != 0) Xx += (w_c2(c2) * dx) * nr;
           if (dy != 0) Xy += (w_c2(c2) * dy) * nr;
         }
       }
     }
+#endif
     double Fx = -gx * rl * Xx - pl * Sx, Fy = -gx * rl * Xy - pl * Sy;
     // moments, Eqs. (5), (17): partial sums of this lane + the other species' lane
     const double Tp = (s ? 0.0 : g0) + ga + gb + gc + gd;
@@ -324,6 +374,9 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       }
     } else {
       // own species: Eq. (6) shifted velocity, Eqs. (2), (3)
+#if defined(TLB_EXP) && (TLB_EXP & 1)
+      f[0] += uHx + uHy + ux + uy + invl;
+#else
       {
         const double vx = ux + Fx * invl, vy = uy + Fy * invl;
         const double usq = 1.0 - 1.5 * (vx * vx + vy * vy);
@@ -349,6 +402,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         gc = relax(gc, w5, vx + vy, usq, d.omega_g);
         gd = relax(gd, w5, -vx + vy, usq, d.omega_g);
       }
+#endif
       if (fluid) {
 #pragma unroll
         for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<double*>(opf + i * planeB), f[i], pol);
