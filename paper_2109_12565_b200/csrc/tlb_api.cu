@@ -211,6 +211,7 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   d.nx = nx; d.ny = ny; d.periodic_y = p->periodic_y ? 1 : 0; d.thermal = p->thermal ? 1 : 0;
   d.px = padded_pitch(nx);
   d.plane = (long long)d.px * (ny + 2);
+  d.row = d.px;
   d.omega = 1.0 / p->tau; d.omega_g = 1.0 / p->tau_g; d.tau = p->tau;
   d.rho0 = p->rho0; d.inv_rho0 = 1.0 / p->rho0;
   d.G12 = p->G12; d.G11a = p->G11a; d.G11r = p->G11r; d.G22a = p->G22a; d.G22r = p->G22r;
@@ -228,8 +229,8 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   if (configure_kernels() != 0) { cudaGetLastError(); delete h; return TLB_ECUDA; }
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field
-  cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.plane * sizeof(double), h->st));
-  cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.plane * sizeof(double), h->st));
+  cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.px * (ny + 2) * sizeof(double), h->st));
+  cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.px * (ny + 2) * sizeof(double), h->st));
   if (check(h) != TLB_OK) { delete h; return TLB_ECUDA; }
   *out = h;
   return TLB_OK;

@@ -73,8 +73,11 @@ __global__ void gather_kernel(const Dev d, const double* __restrict__ S, double*
 
 __global__ void copy_g_kernel(const Dev d, const double* __restrict__ src, double* __restrict__ dst) {
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= 9 * d.plane) return;
-  dst[18 * d.plane + k] = src[18 * d.plane + k];
+  const long long per_row = 9ll * d.px;
+  if (k >= per_row * (d.ny + 2)) return;
+  const long long r = k / per_row, c = k % per_row;  // storage row, (thermal plane, column)
+  const long long o = (18 + c / d.px) * d.plane + r * d.row + c % d.px;
+  dst[o] = src[o];
 }
 
 // Solid in-domain sites with at least one fluid neighbour -> work list of the boundary kernel.
@@ -237,7 +240,7 @@ int launch_gather(const Dev& d, const double* S, double* fA, double* fB, double*
   return 1;
 }
 int launch_copy_g(const Dev& d, const double* Ssrc, double* Sdst, cudaStream_t st) {
-  copy_g_kernel<<<blocks_for(9 * d.plane, 256), 256, 0, st>>>(d, Ssrc, Sdst);
+  copy_g_kernel<<<blocks_for(9ll * d.px * (d.ny + 2), 256), 256, 0, st>>>(d, Ssrc, Sdst);
   return 1;
 }
 int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st) {

@@ -44,7 +44,8 @@ struct Dev {
   int nx, ny;
   int px;                // padded row pitch in doubles (and in bytes of the padded mask)
   int periodic_y, thermal;
-  long long plane;       // (ny + 2) * px, doubles per population plane
+  long long plane;       // doubles between consecutive planes of one node
+  long long row;         // doubles between consecutive rows of one plane
   double omega, omega_g; // 1/tau, 1/tau_g
   double tau;
   double inv_rho0, rho0;
@@ -55,7 +56,7 @@ struct Dev {
   const uint8_t* solidp; // [ny][px]   the same with ghost columns, lattice column x at kXL + x
 
   // offset of lattice node (x, y) inside a plane; x in [-kXL, px - kXL), y in [-1, ny]
-  __host__ __device__ long long at(int x, int y) const { return (long long)(y + 1) * px + kXL + x; }
+  __host__ __device__ long long at(int x, int y) const { return (long long)(y + 1) * row + kXL + x; }
 };
 
 __host__ __device__ inline int padded_pitch(int nx) {

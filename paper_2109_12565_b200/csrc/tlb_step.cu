@@ -153,7 +153,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   auto AT = [&](int xx, int yy) { return ((long long)(yy + 1) * strips_ + blockIdx.x) * 27 * 128 + (xx - x0); };
 #else
   const long long plane = d.plane;
-  const long long planeB = plane * 8, rowB = (long long)px * 8;
+  const long long planeB = plane * 8, rowB = d.row * 8;
   auto AT = [&](int xx, int yy) { return d.at(xx, yy); };
 #endif
   const uint64_t pol = policy_evict_first();  // every line of Sin is dead once read, Sout until the next step
