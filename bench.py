@@ -138,7 +138,7 @@ def run_reference(args, rank):
 def run_ours(args, rank, world):
     import torch
     import torch.distributed as dist
-    from paper_2109_12565_b200 import binding, inputs
+    from paper_2109_12565_b200 import binding, inputs, replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
@@ -152,7 +152,7 @@ def run_ours(args, rank, world):
     nx, ny = cfg["nx"], cfg["ny"]
     sites = nx * ny
     t = binding.TLB(nx, ny, params=binding.params_from_config(cfg), device=dev)
-    t.init(cfg["seed"] + 1000 * rank)
+    t.init(replicas.rank_seed(cfg["seed"], rank))
 
     def barrier():
         if world > 1:
@@ -173,11 +173,7 @@ def run_ours(args, rank, world):
     launches = t.launch_count() - l0
     ms = e0.elapsed_time(e1)
     clocks = sampler.summary()
-    if world > 1:
-        mt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(mt, op=dist.ReduceOp.MAX)
-        ms = float(mt.item())
-    mlups = world * sites * args.steps / ms / 1e3
+    mlups, ms = replicas.aggregate_mlups(sites, args.steps, ms, dev)  # all ranks' updates / max-over-ranks time
 
     # ---- roofline of the dominant (fused) kernel.  Its average launch duration inside the timed region
     # is the step time (CUDA events around the K back-to-back steps above) minus the boundary kernel's
@@ -215,11 +211,8 @@ def run_ours(args, rank, world):
         t.observables()
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - w0) * 1e3
-    if world > 1:
-        mt = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(mt, op=dist.ReduceOp.MAX)
-        e2e_ms = float(mt.item())
-    e2e = {"value": world * sites * e2e_steps / e2e_ms / 1e3, "unit": "MLUPS", "h2d_bytes_per_step": 3 * 8 * sites,
+    e2e_mlups, e2e_ms = replicas.aggregate_mlups(sites, e2e_steps, e2e_ms, dev)
+    e2e = {"value": e2e_mlups, "unit": "MLUPS", "h2d_bytes_per_step": 3 * 8 * sites,
            "d2h_bytes_per_step": 32, "steps": e2e_steps,
            "call": "tlb_set_fields_host + tlb_step(1) + tlb_observables_host per step"}
     del solid_h

@@ -52,9 +52,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   uint32_t done;
   do {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(done)
-        : "r"(smem_u32(bar)), "r"(parity)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(0x989680u)  // suspend-time hint: sleep in hardware instead of spinning
         : "memory");
   } while (!done);
 }
@@ -117,10 +117,10 @@ __device__ __forceinline__ unsigned int count_out(unsigned int* c) {
 __device__ __forceinline__ double pair(double v) { return __shfl_xor_sync(0xffffffffu, v, 1); }  // the other species' lane
 
 // BGK relaxation of one population towards the second-order equilibrium, Eqs. (2), (3) (c_s^2 = 1/3);
-// cu = c_i . u, usq = 1 - 1.5 |u|^2, wd = w_i * density
-__device__ __forceinline__ double relax(double f, double wd, double cu, double usq, double omega) {
-  const double feq = wd * (usq + 3.0 * cu + 4.5 * cu * cu);
-  return f + omega * (feq - f);
+// cu = c_i . u, usq = 1 - 1.5 |u|^2, owd = omega * w_i * density, om1 = 1 - omega:
+// f - (f - f_eq) / tau  =  (1 - omega) f + omega f_eq
+__device__ __forceinline__ double relax(double f, double owd, double cu, double usq, double om1) {
+  return om1 * f + owd * (usq + 3.0 * cu + 4.5 * cu * cu);
 }
 
 }  // namespace
@@ -232,6 +232,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
                k5 = Ga * w_c2(5) + Gr * p_c2(5), k8 = Ga * w_c2(8) + Gr * p_c2(8);
   const double k4d = 2.0 * k4, k5d = 2.0 * k5, k8d = 2.0 * k8;
   const double gx = d.G12 * d.inv_rho0 * d.inv_rho0;  // Eqs. (7), (8): psi^x = rho / rho0 on both factors
+  const double om1 = 1.0 - d.omega, om1g = 1.0 - d.omega_g;
   const double sgn = s ? -1.0 : 1.0;                  // this lane's thermal directions are sgn * {c_1, c_2, c_5, c_6}
 
   // running byte pointers of row y = y0 (advanced by one row per phase-2 iteration)
@@ -380,27 +381,27 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       {
         const double vx = ux + Fx * invl, vy = uy + Fy * invl;
         const double usq = 1.0 - 1.5 * (vx * vx + vy * vy);
-        const double w0 = wq(0) * rl, w1 = wq(1) * rl, w5 = wq(5) * rl;
-        f[0] = relax(f[0], w0, 0.0, usq, d.omega);
-        f[1] = relax(f[1], w1, vx, usq, d.omega);
-        f[2] = relax(f[2], w1, vy, usq, d.omega);
-        f[3] = relax(f[3], w1, -vx, usq, d.omega);
-        f[4] = relax(f[4], w1, -vy, usq, d.omega);
-        f[5] = relax(f[5], w5, vx + vy, usq, d.omega);
-        f[6] = relax(f[6], w5, -vx + vy, usq, d.omega);
-        f[7] = relax(f[7], w5, -vx - vy, usq, d.omega);
-        f[8] = relax(f[8], w5, vx - vy, usq, d.omega);
+        const double w0 = d.omega * (wq(0) * rl), w1 = d.omega * (wq(1) * rl), w5 = d.omega * (wq(5) * rl);
+        f[0] = relax(f[0], w0, 0.0, usq, om1);
+        f[1] = relax(f[1], w1, vx, usq, om1);
+        f[2] = relax(f[2], w1, vy, usq, om1);
+        f[3] = relax(f[3], w1, -vx, usq, om1);
+        f[4] = relax(f[4], w1, -vy, usq, om1);
+        f[5] = relax(f[5], w5, vx + vy, usq, om1);
+        f[6] = relax(f[6], w5, -vx + vy, usq, om1);
+        f[7] = relax(f[7], w5, -vx - vy, usq, om1);
+        f[8] = relax(f[8], w5, vx - vy, usq, om1);
       }
       // own half of the thermal set: Eqs. (16), (18) with u^(H); directions sgn * {c_1, c_2, c_5, c_6}
       if (d.thermal) {
         const double vx = sgn * uHx, vy = sgn * uHy;
         const double usq = 1.0 - 1.5 * (uHx * uHx + uHy * uHy);
-        const double w0 = wq(0) * T, w1 = wq(1) * T, w5 = wq(5) * T;
-        g0 = relax(g0, w0, 0.0, usq, d.omega_g);
-        ga = relax(ga, w1, vx, usq, d.omega_g);
-        gb = relax(gb, w1, vy, usq, d.omega_g);
-        gc = relax(gc, w5, vx + vy, usq, d.omega_g);
-        gd = relax(gd, w5, -vx + vy, usq, d.omega_g);
+        const double w0 = d.omega_g * (wq(0) * T), w1 = d.omega_g * (wq(1) * T), w5 = d.omega_g * (wq(5) * T);
+        g0 = relax(g0, w0, 0.0, usq, om1g);
+        ga = relax(ga, w1, vx, usq, om1g);
+        gb = relax(gb, w1, vy, usq, om1g);
+        gc = relax(gc, w5, vx + vy, usq, om1g);
+        gd = relax(gd, w5, -vx + vy, usq, om1g);
       }
 #endif
       if (fluid) {
@@ -510,7 +511,8 @@ int default_seg_rows(int nx, int ny) {
     const int ctas = strips * segs;
     const int w = (ctas + slots - 1) / slots;
     const double cost = (double)w * (seg + 4);  // rows marched by the busiest slot, incl. warm-up rows
-    const double score = (double)ny * strips / slots / cost;  // 1 = perfect
+    double score = (double)ny * strips / slots / cost;  // 1 = perfect
+    if (w == 1) score *= 0.97;  // a single wave cannot rebalance CTAs that run slow (measured 1-2 % on config 4)
     if (score > best + 1e-9) { best = score; best_seg = seg; }
   }
   return best_seg;

@@ -217,3 +217,59 @@ def test_error_codes(tlbmod):
     n0 = t.launch_count()
     t.step(3)
     assert t.launch_count() == n0 + 6  # fused + boundary kernel per step
+
+
+def test_profile_step_advances_exactly_one_step(tlbmod, oracle_mod):
+    """tlb_profile_step launches each (idempotent) kernel n times and must leave the state one step on."""
+    nx, ny = 130, 40
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4)
+    solid = inputs.post_mask(nx, ny, 3, 3, 10)
+    o, t = _pair(tlbmod, oracle_mod, nx, ny, par, solid)
+    rA, rB, T = inputs.smooth_random_fields(nx, ny, 11, 0.5, -0.5)
+    o.set_fields(rA, rB, T)
+    t.set_fields(rA, rB, T)
+    for n in (1, 3):
+        fused_ms, boundary_ms = t.profile_step(n)
+        o.step(1)
+        assert fused_ms > 0 and boundary_ms > 0
+        assert _maxdiff(o, t) <= TOL
+
+
+def test_full_size_windows_config4(tlbmod, oracle_mod):
+    """BASELINE config 4 at full size (4096x2048, posts, 4000 droplets) in the launch configuration bench.py
+    times: 3 steps on the GPU, compared with the oracle on windows it can compute in seconds.  A site after
+    n steps depends on initial data within 3n cells (2-cell force stencil + 1 cell of streaming per step), so
+    an oracle run on a window is exact farther than 3n cells from the window's artificial edges.  Windows:
+    bottom wall + posts, top wall + posts, the periodic seam in x, a strip edge (x = 128 k) crossing a
+    segment edge, and a bulk window."""
+    import torch
+    cfg = inputs.config(4)
+    nx, ny, steps, m = cfg["nx"], cfg["ny"], 3, 12
+    solid, rA, rB, T = inputs.make_config_inputs(cfg)
+    t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
+    t.init(cfg["seed"])
+    t.step(steps)
+    pops = t.get_populations()
+    ob = t.observables()
+    assert all(np.isfinite(v) for v in ob.values())
+    seg = 114  # rows per segment chosen for this size (2 waves); the window below straddles y = 114 and x = 128
+    windows = [("bottom", np.arange(1000, 1200), np.arange(0, 48), "wall_bottom"),
+               ("top", np.arange(3000, 3200), np.arange(ny - 48, ny), "wall_top"),
+               ("seam", np.r_[np.arange(nx - 80, nx), np.arange(0, 80)], np.arange(900, 960), "bulk"),
+               ("edges", np.arange(128 - 70, 128 + 70), np.arange(seg - 30, seg + 30), "bulk"),
+               ("bulk", np.arange(2000, 2150), np.arange(1500, 1560), "bulk")]
+    for name, xs, ys, kind in windows:
+        sub = np.ix_(ys, xs)
+        par = dict(cfg["params"], periodic_y=1 if kind == "bulk" else 0)
+        o = oracle_mod.Oracle(len(xs), len(ys), **par)
+        o.set_solid(np.ascontiguousarray(solid[sub]))
+        o.set_fields(np.ascontiguousarray(rA[sub]), np.ascontiguousarray(rB[sub]), np.ascontiguousarray(T[sub]))
+        o.step(steps)
+        y_lo = 0 if kind == "wall_bottom" else m
+        y_hi = len(ys) if kind == "wall_top" else len(ys) - m
+        po = o.get_populations()
+        idx_y = torch.as_tensor(ys[y_lo:y_hi], device=pops[0].device)
+        idx_x = torch.as_tensor(xs[m:len(xs) - m], device=pops[0].device)
+        for a, b in zip(po, pops):
+            g = b.index_select(1, idx_y).index_select(2, idx_x).cpu().numpy()
+            assert np.abs(a[:, y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
