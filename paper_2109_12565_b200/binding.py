@@ -11,7 +11,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
-LIB_PATH = os.path.join(_HERE, "libtlb.so")
+LIB_PATH = os.environ.get("TLB_LIB") or os.path.join(_HERE, "libtlb.so")  # TLB_LIB: A/B experiments only
 SOURCES = ["tlb_step.cu", "tlb_aux.cu", "tlb_api.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]

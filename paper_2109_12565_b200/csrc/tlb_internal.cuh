@@ -31,7 +31,10 @@ __host__ __device__ constexpr int opp(int i) { return i == 0 ? 0 : (i <= 4 ? ((i
 __host__ __device__ constexpr double wq(int i) { return i == 0 ? 4.0 / 9.0 : (i <= 4 ? 1.0 / 9.0 : 1.0 / 36.0); }
 
 // fused-kernel geometry (see tlb_step.cu)
-constexpr int kW = 128;                 // strip width = threads per CTA = interior columns per strip
+#ifndef TLB_KW
+#define TLB_KW 128
+#endif
+constexpr int kW = TLB_KW;                 // strip width = threads per CTA = interior columns per strip
 constexpr int kHX = 4;                  // columns fetched beyond the strip on each side (3 needed; 4 keeps 16-byte alignment)
 constexpr int kCopyW = kW + 2 * kHX;    // doubles per plane-row copy
 constexpr int kSlots = 4;               // rows of the 18 fluid planes resident in shared memory

@@ -33,11 +33,8 @@ __device__ __forceinline__ constexpr double p_c2(int c2) {
   return c2 == 1 ? 4.0 / 63.0 : c2 == 2 ? 4.0 / 135.0 : c2 == 4 ? 1.0 / 180.0 : c2 == 5 ? 2.0 / 945.0 : c2 == 8 ? 1.0 / 15120.0 : 0.0;
 }
 
-__device__ __forceinline__ double sum9(const double (&f)[9]) {  // Eq. (4), same order as written
-  double r = f[0];
-#pragma unroll
-  for (int i = 1; i < 9; i++) r += f[i];
-  return r;
+__device__ __forceinline__ double sum9(const double (&f)[9]) {  // Eq. (4); pairwise: depth 4 instead of 8
+  return (((f[0] + f[1]) + (f[2] + f[3])) + ((f[4] + f[5]) + (f[6] + f[7]))) + f[8];
 }
 
 // ---- mbarrier / bulk-copy primitives (PTX; sm_90+ programming model, sm_100a target) ----
@@ -85,15 +82,50 @@ __device__ __forceinline__ void stg_stream(double* a, double v, uint64_t policy)
   asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(a), "d"(v), "l"(policy) : "memory");
 }
 
+// e^x for x <= 0 (the argument of Eq. (12) is -rho / rho0): Cody-Waite reduction x = k ln2 + r,
+// |r| <= ln2 / 2, degree-12 Taylor polynomial (truncation < 2e-16 relative) in Estrin form (short
+// dependency chains), exponent add.  Arguments below -700 are clamped (e^-700 ~ 1e-304 is far below
+// one ulp of the 1 in 1 - e^x).  No special cases: about half the instructions of the library exp,
+// within 1 ulp of it on this range.
+__device__ __forceinline__ double exp_nonpos(double x) {
+  x = fmax(x, -700.0);
+  const double shifter = 6755399441055744.0;  // 1.5 * 2^52: the integer part lands in the low word
+  const double t = fma(x, 1.4426950408889634074, shifter);
+  const int k = __double2loint(t);
+  const double kf = t - shifter;
+  double r = fma(kf, -6.93147180369123816490e-01, x);
+  r = fma(kf, -1.90821492927058770002e-10, r);
+  const double r2 = r * r, r4 = r2 * r2, r8 = r4 * r4;
+  const double a01 = fma(r, 1.0, 1.0), a23 = fma(r, 1.0 / 6.0, 0.5), a45 = fma(r, 1.0 / 120.0, 1.0 / 24.0),
+               a67 = fma(r, 1.0 / 5040.0, 1.0 / 720.0), a89 = fma(r, 1.0 / 362880.0, 1.0 / 40320.0),
+               aab = fma(r, 1.0 / 39916800.0, 1.0 / 3628800.0);
+  const double b0 = fma(r2, a23, a01), b1 = fma(r2, a67, a45), b2 = fma(r2, aab, a89);
+  const double c0 = fma(r4, b1, b0), c1 = fma(r4, 1.0 / 479001600.0, b2);
+  const double p = fma(r8, c1, c0);
+  return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// 1 / a for normal a > 0: hardware seed (20 bits) and two Newton steps; within 1 ulp, no slow path
+__device__ __forceinline__ double rcp_pos(double a) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(a));
+  double e = fma(-a, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-a, y, 1.0);
+  y = fma(y, e, y);
+  return y;
+}
+
 __device__ __forceinline__ int wrap_row(int r, int ny) {
   r %= ny;
   return r < 0 ? r + ny : r;
 }
 
 #ifndef TLB_PREF_D
-#define TLB_PREF_D 4
+#define TLB_PREF_D 0
 #endif
-constexpr int kPrefetchRows = TLB_PREF_D;  // rows the HBM -> L2 prefetch runs ahead of the shared-memory copy
+constexpr int kPrefetchRows = TLB_PREF_D;  // rows an optional HBM -> L2 prefetch runs ahead of the copies (0 = off: measured 3 % faster)
+constexpr int kCtasPerSM = 256 / kW;     // shared memory allows 2 CTAs of 128 columns (or 1 of 256) per SM
 constexpr int kThreads = 2 * kW;       // two threads per lattice column: lane 2k = species A, 2k+1 = species B
 constexpr int kWarps = kThreads / 32;  // 8
 constexpr int kWC = 16;                // lattice columns per warp
@@ -131,7 +163,7 @@ __device__ __forceinline__ double relax(double f, double owd, double cu, double 
 // set: s = 0 takes g_0, g_1, g_2, g_5, g_6, s = 1 the opposite directions g_3, g_4, g_7, g_8, so both
 // lanes run the same code on (c_i, u) and (-c_i, -u).  Partial sums (j, F, T) cross by one shuffle.
 template <int MODE, bool PERIODIC>
-__global__ void __launch_bounds__(kThreads, 2)
+__global__ void __launch_bounds__(kThreads, kCtasPerSM)
 fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ Sout, int seg_rows,
              double* __restrict__ oRA, double* __restrict__ oRB, double* __restrict__ oUx, double* __restrict__ oUy,
              double* __restrict__ oT) {
@@ -146,16 +178,8 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   const int x = xw + 2 + k;                   // phase-2 column of this lane pair
   const int y0 = blockIdx.y * seg_rows;
   const int y1 = min(ny, y0 + seg_rows);
-#if defined(TLB_EXP) && (TLB_EXP & 2)
-  const int strips_ = gridDim.x;          // EXPERIMENT: (row, strip)-tiled layout, timing only
-  const long long plane = 128;
-  const long long planeB = plane * 8, rowB = (long long)strips_ * 27 * 128 * 8;
-  auto AT = [&](int xx, int yy) { return ((long long)(yy + 1) * strips_ + blockIdx.x) * 27 * 128 + (xx - x0); };
-#else
   const long long plane = d.plane;
   const long long planeB = plane * 8, rowB = d.row * 8;
-  auto AT = [&](int xx, int yy) { return d.at(xx, yy); };
-#endif
   const uint64_t pol = policy_evict_first();  // every line of Sin is dead once read, Sout until the next step
 
   if (t == 0) {
@@ -180,7 +204,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     }
     uint64_t* bar = &sm.full[q & 3];
     mbar_expect_tx(bar, 18u * kCopyW * 8u);
-    const long long o0 = AT(x0 - kHX, rr), om = AT(x0 - kHX, rm), op = AT(x0 - kHX, rp);
+    const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
 #pragma unroll
     for (int l = 0; l < 2; l++)
 #pragma unroll
@@ -199,7 +223,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       if (rm < 0) rm = ny - 1;
       if (rp >= ny) rp = 0;
     }
-    const long long o0 = AT(x0 - kHX, rr), om = AT(x0 - kHX, rm), op = AT(x0 - kHX, rp);
+    const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
     const int np = (d.thermal && q >= 2 && q < q_end - 2) ? 27 : 18;  // g only for rows that reach phase 2
 #pragma unroll
     for (int p = 0; p < 27; p++) {
@@ -236,9 +260,9 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   const double sgn = s ? -1.0 : 1.0;                  // this lane's thermal directions are sgn * {c_1, c_2, c_5, c_6}
 
   // running byte pointers of row y = y0 (advanced by one row per phase-2 iteration)
-  const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + AT(x, y0));   // g_{i + 2s}
-  char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + AT(x, y0));                    // own species
-  char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + AT(x, y0));             // own thermal half
+  const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + d.at(x, y0));   // g_{i + 2s}
+  char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + d.at(x, y0));                    // own species
+  char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + d.at(x, y0));             // own thermal half
   const int co = s ? 8 : -8;                                                                    // x - c_x of c_1 / c_3
 
   // thermal populations of (x, y).  Lane s = 0 reads
@@ -286,12 +310,8 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         double f[9];
 #pragma unroll
         for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
-#if defined(TLB_EXP) && (TLB_EXP & 4)
-        rl = f[0] + f[8]; pl = rl;
-#else
         rl = sum9(f);
-        pl = d.rho0 * (1.0 - exp(-rl * d.inv_rho0));
-#endif
+        pl = d.rho0 * (1.0 - exp_nonpos(-rl * d.inv_rho0));
       }
       rho_r[rq][c][s] = rl;
       psi_r[rq][c][s] = pl;
@@ -318,8 +338,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     const bool fluid = x < nx && !flag[rq0][cc];
     const double rl = rho_r[rq0][cc][s], rn = rho_r[rq0][cc][1 - s], pl = psi_r[rq0][cc][s];
     // force sums over the 5x5 neighbourhood: cross (w, other species' rho), self (G_a w + G_r p, own psi^s)
-    double Xx = 0, Xy = 0, Sx = 0, Sy = 0;
-#if !defined(TLB_EXP) || !(TLB_EXP & 1)
+    double Xx = 0, Xy = 0, Sx = 0, Sy = 0, Sx2 = 0, Sy2 = 0;  // S = S + S2: two dependency chains per component
 #pragma unroll
     for (int dy = -2; dy <= 2; dy++) {
       const int sl = (q + kRingRows - 2 + dy) % kRingRows;
@@ -330,10 +349,12 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         const double kk = c2 == 1 ? k1 : c2 == 2 ? k2 : c2 == 4 ? k4 : c2 == 5 ? k5 : k8;      // |component| = 1
         const double kd = c2 == 4 ? k4d : c2 == 5 ? k5d : k8d;                                  // |component| = 2
         const double ns = psi_r[sl][cc + dx][s];
-        if (dx > 0) Sx += (dx == 1 ? kk : kd) * ns;
-        if (dx < 0) Sx -= (dx == -1 ? kk : kd) * ns;
-        if (dy > 0) Sy += (dy == 1 ? kk : kd) * ns;
-        if (dy < 0) Sy -= (dy == -1 ? kk : kd) * ns;
+        double& ax = dy > 0 ? Sx2 : Sx;
+        double& ay = dx > 0 ? Sy2 : Sy;
+        if (dx > 0) ax += (dx == 1 ? kk : kd) * ns;
+        if (dx < 0) ax -= (dx == -1 ? kk : kd) * ns;
+        if (dy > 0) ay += (dy == 1 ? kk : kd) * ns;
+        if (dy < 0) ay -= (dy == -1 ? kk : kd) * ns;
         if (c2 <= 2) {
           const double nr = rho_r[sl][cc + dx][1 - s];
           if (dx != 0) Xx += (w_c2(c2) * dx) * nr;
@@ -341,20 +362,21 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         }
       }
     }
-#endif
+    Sx += Sx2;
+    Sy += Sy2;
     double Fx = -gx * rl * Xx - pl * Sx, Fy = -gx * rl * Xy - pl * Sy;
     // moments, Eqs. (5), (17): partial sums of this lane + the other species' lane
     const double Tp = (s ? 0.0 : g0) + ga + gb + gc + gd;
     const double T = Tp + pair(Tp);
-    const double jxl = f[1] - f[3] + f[5] - f[6] - f[7] + f[8];
-    const double jyl = f[2] - f[4] + f[5] + f[6] - f[7] - f[8];
+    const double jxl = ((f[1] - f[3]) + (f[5] - f[6])) + (f[8] - f[7]);
+    const double jyl = ((f[2] - f[4]) + (f[5] - f[7])) + (f[6] - f[8]);
     const double jx = jxl + pair(jxl), jy = jyl + pair(jyl);
     // Eq. (22) buoyancy (R12) and the x-acceleration extension
     const double dT = d.thermal ? (T - d.T_ref) : 0.0;
     Fy += rl * d.alpha_g * dT;
     Fx += rl * d.body_ax;
     const double rho = rl + rn;
-    const double inv = 1.0 / rho, invl = d.tau / rl;
+    const double inv = rcp_pos(rho), invl = d.tau * rcp_pos(rl);
     const double ux = jx * inv, uy = jy * inv;                      // Eq. (5)
     const double Ftx = Fx + pair(Fx), Fty = Fy + pair(Fy);
     const double uHx = (jx + 0.5 * Ftx) * inv, uHy = (jy + 0.5 * Fty) * inv;  // L139
@@ -375,9 +397,6 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       }
     } else {
       // own species: Eq. (6) shifted velocity, Eqs. (2), (3)
-#if defined(TLB_EXP) && (TLB_EXP & 1)
-      f[0] += uHx + uHy + ux + uy + invl;
-#else
       {
         const double vx = ux + Fx * invl, vy = uy + Fy * invl;
         const double usq = 1.0 - 1.5 * (vx * vx + vy * vy);
@@ -403,7 +422,6 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
         gc = relax(gc, w5, vx + vy, usq, om1g);
         gd = relax(gd, w5, -vx + vy, usq, om1g);
       }
-#endif
       if (fluid) {
 #pragma unroll
         for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<double*>(opf + i * planeB), f[i], pol);
@@ -499,7 +517,7 @@ int configure_kernels() {
 // Rows per CTA segment: strips x segments should fill whole waves of 2 CTAs per SM on 148 SMs with
 // as few segments as possible (each segment re-reads 4 warm-up rows), never below 16 rows.
 int default_seg_rows(int nx, int ny) {
-  const int strips = (nx + kW - 1) / kW, slots = 2 * 148;
+  const int strips = (nx + kW - 1) / kW, slots = kCtasPerSM * 148;
   int best_seg = ny;
   double best = -1.0;
   for (int waves = 1; waves <= 4; waves++) {
