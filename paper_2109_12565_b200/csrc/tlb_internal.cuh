@@ -34,7 +34,7 @@ __host__ __device__ constexpr double wq(int i) { return i == 0 ? 4.0 / 9.0 : (i 
 #ifndef TLB_KW
 #define TLB_KW 128
 #endif
-constexpr int kW = TLB_KW;                 // strip width = threads per CTA = interior columns per strip
+constexpr int kW = TLB_KW;              // strip width = lattice columns per CTA (two threads per column)
 constexpr int kHX = 4;                  // columns fetched beyond the strip on each side (3 needed; 4 keeps 16-byte alignment)
 constexpr int kCopyW = kW + 2 * kHX;    // doubles per plane-row copy
 constexpr int kSlots = 4;               // rows of the 18 fluid planes resident in shared memory
