@@ -112,7 +112,9 @@ int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, 
 int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g);
 
 /* Advance n >= 0 time steps (n = 0 is a no-op): per step one fused force+collide+stream kernel and
- * one wall/obstacle boundary kernel. */
+ * one wall/obstacle boundary kernel.  Whole blocks of 16 steps are replayed from a CUDA graph captured on
+ * first use (one launch instead of 32; matters for launch-bound lattices); the rest is launched kernel by
+ * kernel.  Set the environment variable TLB_NO_GRAPH to disable the graphs. */
 int tlb_step(tlb_handle* h, int64_t n);
 
 /* Measurement aid: advance ONE step, launching the fused kernel n (1..4096) times back to back on the

@@ -29,6 +29,11 @@ struct tlb_handle {
   bool has_state;
   cudaError_t err;
   int64_t launches;
+  // CUDA graphs of kGraphSteps consecutive steps, one per starting buffer parity (launch-bound lattices)
+  cudaStream_t cap_stream;
+  cudaGraphExec_t gexec[2];
+  int64_t g_launches[2];
+  bool use_graph;
 };
 
 namespace {
@@ -78,6 +83,45 @@ int cu(tlb_handle* h, cudaError_t e) {
   return h->err == cudaSuccess ? TLB_OK : TLB_ECUDA;
 }
 
+constexpr int kGraphSteps = 16;
+
+void drop_graphs(tlb_handle* h) {
+  for (int k = 0; k < 2; k++)
+    if (h->gexec[k]) { cudaGraphExecDestroy(h->gexec[k]); h->gexec[k] = nullptr; }
+}
+
+// Capture kGraphSteps steps starting from buffer parity `cur` (kernel arguments are baked in: the
+// graph is dropped whenever the boundary work list changes).  Returns false if capture is not possible;
+// the caller then launches the kernels one by one.
+bool ensure_graph(tlb_handle* h, int cur) {
+  if (h->gexec[cur]) return true;
+  if (!h->use_graph || !h->cap_stream) return false;
+  if (cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+    cudaGetLastError();
+    h->use_graph = false;
+    return false;
+  }
+  int64_t n = 0;
+  int c = cur;
+  for (int t = 0; t < kGraphSteps; t++) {
+    n += launch_step(h->d, h->S[c], h->S[1 - c], h->seg_rows, h->cap_stream);
+    n += launch_boundary(h->d, h->S[1 - c], h->sites, h->n_sites, h->cap_stream);
+    c = 1 - c;
+  }
+  cudaGraph_t g = nullptr;
+  cudaError_t e = cudaStreamEndCapture(h->cap_stream, &g);
+  if (e == cudaSuccess) e = cudaGraphInstantiate(&h->gexec[cur], g, 0);
+  if (g) cudaGraphDestroy(g);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    h->gexec[cur] = nullptr;
+    h->use_graph = false;
+    return false;
+  }
+  h->g_launches[cur] = n;
+  return true;
+}
+
 // After the mask changed: rebuild the boundary work list (count comes back to size the launch).
 int rebuild_links(tlb_handle* h) {
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);
@@ -85,6 +129,7 @@ int rebuild_links(tlb_handle* h) {
   cu(h, cudaMemcpyAsync(&c, h->count, sizeof(int), cudaMemcpyDeviceToHost, h->st));
   cu(h, cudaStreamSynchronize(h->st));
   h->n_sites = c;
+  drop_graphs(h);
   h->has_state = false;
   return check(h);
 }
@@ -226,12 +271,20 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   if (const char* e = std::getenv("TLB_SEG_ROWS")) { const int v = std::atoi(e); if (v > 0) seg = v; }
   if (seg > ny) seg = ny;
   h->seg_rows = seg;
-  if (configure_kernels() != 0) { cudaGetLastError(); delete h; return TLB_ECUDA; }
+  h->gexec[0] = h->gexec[1] = nullptr;
+  h->cap_stream = nullptr;
+  h->use_graph = std::getenv("TLB_NO_GRAPH") == nullptr;
+  if (h->use_graph && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+    cudaGetLastError();
+    h->cap_stream = nullptr;
+    h->use_graph = false;
+  }
+  if (configure_kernels() != 0) { cudaGetLastError(); tlb_destroy(h); return TLB_ECUDA; }
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field
   cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.px * (ny + 2) * sizeof(double), h->st));
   cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.px * (ny + 2) * sizeof(double), h->st));
-  if (check(h) != TLB_OK) { delete h; return TLB_ECUDA; }
+  if (check(h) != TLB_OK) { tlb_destroy(h); return TLB_ECUDA; }
   *out = h;
   return TLB_OK;
 }
@@ -239,6 +292,8 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
 int tlb_destroy(tlb_handle* h) {
   if (!h) return TLB_EINVAL;
   cudaStreamSynchronize(h->st);
+  drop_graphs(h);
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   delete h;
   return TLB_OK;
 }
@@ -338,7 +393,14 @@ int tlb_step(tlb_handle* h, int64_t n) {
   if (!h || n < 0) return TLB_EINVAL;
   if (!h->has_state) return TLB_ESTATE;
   if (h->err != cudaSuccess) return TLB_ECUDA;
-  for (int64_t t = 0; t < n; t++) {
+  int64_t t = 0;
+  // whole blocks of kGraphSteps steps replay a captured graph (one launch instead of 2 * kGraphSteps)
+  while (n - t >= kGraphSteps && ensure_graph(h, h->cur)) {
+    if (cu(h, cudaGraphLaunch(h->gexec[h->cur], h->st)) != TLB_OK) return TLB_ECUDA;
+    h->launches += h->g_launches[h->cur];
+    t += kGraphSteps;  // an even number of steps: h->cur is unchanged
+  }
+  for (; t < n; t++) {
     double* in = h->S[h->cur];
     double* out = h->S[1 - h->cur];
     h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);

@@ -515,7 +515,12 @@ int configure_kernels() {
 }
 
 // Rows per CTA segment: strips x segments should fill whole waves of 2 CTAs per SM on 148 SMs with
-// as few segments as possible (each segment re-reads 4 warm-up rows), never below 16 rows.
+// as few segments as possible (each segment re-reads 4 warm-up rows), never below kMinSegRows rows
+// (small lattices are bound by the latency of the serial march, not by the redundant rows).
+#ifndef TLB_MIN_SEG
+#define TLB_MIN_SEG 2
+#endif
+constexpr int kMinSegRows = TLB_MIN_SEG;
 int default_seg_rows(int nx, int ny) {
   const int strips = (nx + kW - 1) / kW, slots = kCtasPerSM * 148;
   int best_seg = ny;
@@ -524,7 +529,7 @@ int default_seg_rows(int nx, int ny) {
     int segs = waves * slots / strips;
     if (segs < 1) segs = 1;
     int seg = (ny + segs - 1) / segs;
-    if (seg < 16) seg = ny < 16 ? ny : 16;
+    if (seg < kMinSegRows) seg = ny < kMinSegRows ? ny : kMinSegRows;
     segs = (ny + seg - 1) / seg;
     const int ctas = strips * segs;
     const int w = (ctas + slots - 1) / slots;

@@ -273,3 +273,24 @@ def test_full_size_windows_config4(tlbmod, oracle_mod):
         for a, b in zip(po, pops):
             g = b.index_select(1, idx_y).index_select(2, idx_x).cpu().numpy()
             assert np.abs(a[:, y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
+
+
+def test_table_b8b_on_the_gpu(tlbmod):
+    """The paper's own printed numbers through the CUDA path: rows of Table B.8(b) (PAPER.md L497-508,
+    tests/golden/table_b8b.txt), 128x2 doubly periodic, Table B.8 parameters, two-layer start (R15),
+    5e4 steps, max / min of the first component's density."""
+    import os
+    golden = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "table_b8b.txt")
+    rows = [tuple(map(float, ln.split())) for ln in open(golden) if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 18
+    first = np.arange(128)[None, :].repeat(2, 0) <= 64
+    for g_print, g_run, rmax, rmin in rows:
+        t = tlbmod.TLB(128, 2, tau=1.0, tau_g=1.0, rho0=0.83, G12=g_run, G11a=-9.0, G11r=8.1, G22a=-8.0, G22r=7.1,
+                       periodic_y=1, thermal=0, alpha_g=0.0, T_ref=0.0, T_bottom=0.0, T_top=0.0)
+        t.set_fields(np.where(first, 1.4, 0.1), np.where(first, 0.1, 1.4), np.zeros((2, 128)))
+        t.step(50000)
+        rA = t.fields()[0].cpu().numpy()
+        assert abs(rA.max() / rmax - 1) < 1e-4 and abs(rA.min() / rmin - 1) < 1e-4, (g_print, rA.max(), rA.min())
+        if g_run >= 0.45 or g_run <= 0.10:
+            assert abs(rA.max() / rmax - 1) < 2e-6 and abs(rA.min() / rmin - 1) < 2e-6, (g_print, rA.max(), rA.min())
+        t.close()
