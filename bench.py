@@ -151,7 +151,8 @@ def run_ours(args, rank, world):
     cfg = inputs.config(args.config)
     nx, ny = cfg["nx"], cfg["ny"]
     sites = nx * ny
-    t = binding.TLB(nx, ny, params=binding.params_from_config(cfg), device=dev)
+    alg_bytes = ALG_BYTES_PER_SITE * args.pop_precision // 64  # 432 B (fp64 storage) or 216 B (fp32 storage)
+    t = binding.TLB(nx, ny, params=binding.params_from_config(cfg), device=dev, pop_precision=args.pop_precision)
     t.init(replicas.rank_seed(cfg["seed"], rank))
 
     def barrier():
@@ -185,12 +186,12 @@ def run_ours(args, rank, world):
     step_ms = ms / args.steps
     fused_ms = step_ms - boundary_ms
     peak, peak_src = measured_peak()
-    achieved = ALG_BYTES_PER_SITE * sites / fused_ms / 1e6  # GB/s
+    achieved = alg_bytes * sites / fused_ms / 1e6  # GB/s
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(cfg["name"]), "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false>",
+                "traffic": committed_traffic(cfg["name"]) if args.pop_precision == 64 else None, "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false>",
                 "kernel_ms": fused_ms, "kernel_ms_isolated": iso_ms, "boundary_kernel_ms": boundary_ms,
                 "method": "kernel_ms = ms_per_step - boundary_kernel_ms (CUDA events on the launch stream)",
-                "alg_bytes_per_launch": ALG_BYTES_PER_SITE * sites, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "alg_bytes_per_launch": alg_bytes * sites, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                 "kernel_share_of_step": fused_ms / step_ms}
     ob = t.observables()
     finite = all(v == v and abs(v) != float("inf") for v in ob.values())
@@ -233,12 +234,12 @@ def run_ours(args, rank, world):
             "warmup": max(3, args.warmup), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": cfg["name"], "nx": nx, "ny": ny, "droplets": cfg["init"]["n_droplets"],
-                       "posts": list(cfg["posts"]), "state_bytes": 216 * sites,
+                       "posts": list(cfg["posts"]), "state_bytes": alg_bytes // 2 * sites, "pop_precision": args.pop_precision,
                        "l2": "state (%.2f GB per buffer) exceeds the 126 MB L2; no flush needed" % (216 * sites / 1e9)
                        if 216 * sites > 4 * 126e6 else "state fits in L2: HBM figures are not meaningful",
                        "parallelism": "replicas x%d" % world, "finite": finite, "mass_A": ob["mass_A"], "Nu": ob["Nu"]},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
-            "effective_GBs": ALG_BYTES_PER_SITE * mlups / 1e3, "roofline_frac_whole_step": ALG_BYTES_PER_SITE * mlups / 1e3 / peak / world}))
+            "effective_GBs": alg_bytes * mlups / 1e3, "roofline_frac_whole_step": alg_bytes * mlups / 1e3 / peak / world}))
     if world > 1:
         dist.destroy_process_group()
 
@@ -251,6 +252,8 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pop-precision", type=int, default=64, choices=[64, 32],
+                    help="storage of the populations in HBM (32: bandwidth study of BASELINE config 5; arithmetic stays fp64)")
     args = ap.parse_args()
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     if args.impl == "reference":

@@ -69,7 +69,8 @@ typedef struct tlb_params {
   int32_t periodic_y;                 /* 0: walls (default); 1: periodic in y (L147, L284-302)              */
   int32_t thermal;                    /* THERMAL switch, L314: 0 leaves g untouched and uses T = T_ref      */
   int32_t post_w, post_h, post_period;/* structured rough walls used by tlb_init (R19); 0,0,0 = smooth      */
-  int32_t pop_precision;              /* 64 (only value accepted in this round)                             */
+  int32_t pop_precision;              /* storage of the populations in HBM: 64 (default) or 32 (bandwidth   */
+                                      /* study of BASELINE config 5; the arithmetic stays fp64)             */
   int32_t reserved;
 } tlb_params;
 

@@ -14,7 +14,8 @@ struct tlb_handle {
   Dev d;
   tlb_params p;
   cudaStream_t st;
-  double* S[2];       // population buffers (pull form), 27 planes each
+  void* S[2];         // population buffers (pull form), 27 planes each, double or float (pop_precision)
+  double* stage;      // [27][ny][nx] doubles for the *_host population calls when the buffers are float
   double* fld[5];     // rho_A, rho_B, u_x, u_y, T scratch planes
   uint8_t* solid;
   uint8_t* solidp;     // padded copy for the fused kernel
@@ -41,15 +42,18 @@ namespace {
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
 struct Layout {
-  size_t S0, S1, fld, solid, solidp, sites, count, partials, out4, centres, total;
+  size_t S0, S1, stage, fld, solid, solidp, sites, count, partials, out4, centres, total;
 };
 
 Layout make_layout(int nx, int ny, const tlb_params* p) {
   const size_t n = (size_t)nx * ny, px = (size_t)padded_pitch(nx), plane = px * (ny + 2);
   Layout L;
   size_t o = 0;
-  L.S0 = o; o = align_up(o + 27 * plane * sizeof(double));
-  L.S1 = o; o = align_up(o + 27 * plane * sizeof(double));
+  const size_t esz = p->pop_precision == 32 ? sizeof(float) : sizeof(double);
+  L.S0 = o; o = align_up(o + 27 * plane * esz);
+  L.S1 = o; o = align_up(o + 27 * plane * esz);
+  // fp64 buffers double as the staging area of the *_host population calls; fp32 buffers are too small
+  L.stage = o; if (p->pop_precision == 32) o = align_up(o + 27 * n * sizeof(double));
   L.fld = o; o = align_up(o + 5 * n * sizeof(double));
   L.solid = o; o = align_up(o + n);
   L.solidp = o; o = align_up(o + px * ny);
@@ -67,7 +71,7 @@ bool params_ok(int nx, int ny, const tlb_params* p) {
   if ((long long)padded_pitch(nx) * (ny + 2) * 27 >= (1ll << 40)) return false;
   if ((long long)nx * ny >= (1ll << 31)) return false;
   if (!(p->tau > 0.5) || !(p->tau_g > 0.5) || !(p->rho0 > 0.0)) return false;
-  if (p->pop_precision != 64 && p->pop_precision != 0) return false;
+  if (p->pop_precision != 64 && p->pop_precision != 32 && p->pop_precision != 0) return false;
   if (p->n_droplets < 0 || p->post_w < 0 || p->post_h < 0 || p->post_period < 0) return false;
   const bool posts = p->post_w > 0 && p->post_h > 0 && p->post_period > 0;
   if (posts && (p->periodic_y || 2 * p->post_h >= ny || p->post_w > p->post_period)) return false;
@@ -242,8 +246,9 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   char* w = static_cast<char*>(workspace);
   h->p = *p;
   h->st = static_cast<cudaStream_t>(stream);
-  h->S[0] = reinterpret_cast<double*>(w + L.S0);
-  h->S[1] = reinterpret_cast<double*>(w + L.S1);
+  h->S[0] = w + L.S0;
+  h->S[1] = w + L.S1;
+  h->stage = p->pop_precision == 32 ? reinterpret_cast<double*>(w + L.stage) : nullptr;
   for (int k = 0; k < 5; k++) h->fld[k] = reinterpret_cast<double*>(w + L.fld) + (size_t)k * nx * ny;
   h->solid = reinterpret_cast<uint8_t*>(w + L.solid);
   h->solidp = reinterpret_cast<uint8_t*>(w + L.solidp);
@@ -255,6 +260,7 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   Dev& d = h->d;
   d.nx = nx; d.ny = ny; d.periodic_y = p->periodic_y ? 1 : 0; d.thermal = p->thermal ? 1 : 0;
   d.px = padded_pitch(nx);
+  d.prec = p->pop_precision == 32 ? 32 : 64;
   d.plane = (long long)d.px * (ny + 2);
   d.row = d.px;
   d.omega = 1.0 / p->tau; d.omega_g = 1.0 / p->tau_g; d.tau = p->tau;
@@ -282,8 +288,8 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   if (configure_kernels() != 0) { cudaGetLastError(); tlb_destroy(h); return TLB_ECUDA; }
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field
-  cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.px * (ny + 2) * sizeof(double), h->st));
-  cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.px * (ny + 2) * sizeof(double), h->st));
+  cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.px * (ny + 2) * (d.prec == 32 ? sizeof(float) : sizeof(double)), h->st));
+  cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.px * (ny + 2) * (d.prec == 32 ? sizeof(float) : sizeof(double)), h->st));
   if (check(h) != TLB_OK) { tlb_destroy(h); return TLB_ECUDA; }
   *out = h;
   return TLB_OK;
@@ -363,7 +369,7 @@ int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g) {
 int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, const double* g) {
   if (!h || !fA || !fB || !g) return TLB_EINVAL;
   const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
-  double* stage = h->S[1 - h->cur];
+  double* stage = h->stage ? h->stage : static_cast<double*>(h->S[1 - h->cur]);
   cu(h, cudaMemcpyAsync(stage, fA, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
   cu(h, cudaMemcpyAsync(stage + n9, fB, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
   cu(h, cudaMemcpyAsync(stage + 2 * n9, g, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
@@ -379,12 +385,12 @@ int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g) {
   if (!h || !fA || !fB || !g) return TLB_EINVAL;
   if (!h->has_state) return TLB_ESTATE;
   const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
-  double* stage = h->S[1 - h->cur];
+  double* stage = h->stage ? h->stage : static_cast<double*>(h->S[1 - h->cur]);
   h->launches += launch_gather(h->d, h->S[h->cur], stage, stage + n9, stage + 2 * n9, h->st);
   cu(h, cudaMemcpyAsync(fA, stage, n9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
   cu(h, cudaMemcpyAsync(fB, stage + n9, n9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
   cu(h, cudaMemcpyAsync(g, stage + 2 * n9, n9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
-  if (!h->d.thermal) h->launches += launch_copy_g(h->d, h->S[h->cur], stage, h->st);
+  if (!h->d.thermal && !h->stage) h->launches += launch_copy_g(h->d, h->S[h->cur], h->S[1 - h->cur], h->st);
   cu(h, cudaStreamSynchronize(h->st));
   return check(h);
 }
@@ -401,8 +407,8 @@ int tlb_step(tlb_handle* h, int64_t n) {
     t += kGraphSteps;  // an even number of steps: h->cur is unchanged
   }
   for (; t < n; t++) {
-    double* in = h->S[h->cur];
-    double* out = h->S[1 - h->cur];
+    void* in = h->S[h->cur];
+    void* out = h->S[1 - h->cur];
     h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);
     h->launches += launch_boundary(h->d, out, h->sites, h->n_sites, h->st);
     h->cur = 1 - h->cur;
@@ -419,8 +425,8 @@ int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundar
   // to back between two events and the state advances by exactly one step.
   cudaEvent_t ev[3];
   for (auto& e : ev) cu(h, cudaEventCreate(&e));
-  double* in = h->S[h->cur];
-  double* out = h->S[1 - h->cur];
+  void* in = h->S[h->cur];
+  void* out = h->S[1 - h->cur];
   cu(h, cudaEventRecord(ev[0], h->st));
   for (int64_t t = 0; t < n; t++) h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);
   cu(h, cudaEventRecord(ev[1], h->st));

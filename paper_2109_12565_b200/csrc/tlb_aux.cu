@@ -18,9 +18,9 @@ __device__ __forceinline__ bool fluid_at(const Dev& d, int x, int y) {
 // One thread per node of the padded lattice (rows -1..ny, columns -kGhost..nx+kGhost-1; ghost columns
 // are the periodic images).  S_i(s) = f_i(s + c_i) when s + c_i is a fluid site (Eq. (1) read
 // backwards), else 0.  RHO = true: f_i = w_i * field (R14).
-template <bool RHO>
+template <bool RHO, typename ST>
 __global__ void scatter_kernel(const Dev d, const double* __restrict__ a, const double* __restrict__ b,
-                               const double* __restrict__ c, double* __restrict__ S) {
+                               const double* __restrict__ c, ST* __restrict__ S) {
   const int nx = d.nx, ny = d.ny, wpad = nx + 2 * kGhost;
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= (long long)wpad * (ny + 2)) return;
@@ -44,14 +44,15 @@ __global__ void scatter_kernel(const Dev d, const double* __restrict__ a, const 
         va = a[i * n + q]; vb = b[i * n + q]; vc = c[i * n + q];
       }
     }
-    S[i * d.plane + o] = va;
-    S[(9 + i) * d.plane + o] = vb;
-    S[(18 + i) * d.plane + o] = vc;
+    S[i * d.plane + o] = (ST)va;
+    S[(9 + i) * d.plane + o] = (ST)vb;
+    S[(18 + i) * d.plane + o] = (ST)vc;
   }
 }
 
 // f_i(x, t) = S_i(x - c_i); 0 on solid sites.
-__global__ void gather_kernel(const Dev d, const double* __restrict__ S, double* __restrict__ a,
+template <typename ST>
+__global__ void gather_kernel(const Dev d, const ST* __restrict__ S, double* __restrict__ a,
                               double* __restrict__ b, double* __restrict__ c) {
   const int nx = d.nx, ny = d.ny;
   const size_t n = (size_t)nx * ny;
@@ -65,13 +66,14 @@ __global__ void gather_kernel(const Dev d, const double* __restrict__ S, double*
     int sy = y - cy(i);
     if (d.periodic_y) sy = wrapi(sy, ny);
     const long long o = d.at(sx, sy);
-    if (a) a[i * n + q] = sol ? 0.0 : S[i * d.plane + o];
-    if (b) b[i * n + q] = sol ? 0.0 : S[(9 + i) * d.plane + o];
-    if (c) c[i * n + q] = sol ? 0.0 : S[(18 + i) * d.plane + o];
+    if (a) a[i * n + q] = sol ? 0.0 : (double)S[i * d.plane + o];
+    if (b) b[i * n + q] = sol ? 0.0 : (double)S[(9 + i) * d.plane + o];
+    if (c) c[i * n + q] = sol ? 0.0 : (double)S[(18 + i) * d.plane + o];
   }
 }
 
-__global__ void copy_g_kernel(const Dev d, const double* __restrict__ src, double* __restrict__ dst) {
+template <typename ST>
+__global__ void copy_g_kernel(const Dev d, const ST* __restrict__ src, ST* __restrict__ dst) {
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long per_row = 9ll * d.px;
   if (k >= per_row * (d.ny + 2)) return;
@@ -227,20 +229,28 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
 
 }  // namespace
 
-int launch_scatter(const Dev& d, const double* fA, const double* fB, const double* g, double* S, cudaStream_t st) {
-  scatter_kernel<false><<<blocks_for((long long)(d.nx + 2 * kGhost) * (d.ny + 2), 128), 128, 0, st>>>(d, fA, fB, g, S);
+int launch_scatter(const Dev& d, const double* fA, const double* fB, const double* g, void* S, cudaStream_t st) {
+  const unsigned nb = blocks_for((long long)(d.nx + 2 * kGhost) * (d.ny + 2), 128);
+  if (d.prec == 32) scatter_kernel<false, float><<<nb, 128, 0, st>>>(d, fA, fB, g, static_cast<float*>(S));
+  else scatter_kernel<false, double><<<nb, 128, 0, st>>>(d, fA, fB, g, static_cast<double*>(S));
   return 1;
 }
-int launch_set_fields(const Dev& d, const double* rhoA, const double* rhoB, const double* T, double* S, cudaStream_t st) {
-  scatter_kernel<true><<<blocks_for((long long)(d.nx + 2 * kGhost) * (d.ny + 2), 128), 128, 0, st>>>(d, rhoA, rhoB, T, S);
+int launch_set_fields(const Dev& d, const double* rhoA, const double* rhoB, const double* T, void* S, cudaStream_t st) {
+  const unsigned nb = blocks_for((long long)(d.nx + 2 * kGhost) * (d.ny + 2), 128);
+  if (d.prec == 32) scatter_kernel<true, float><<<nb, 128, 0, st>>>(d, rhoA, rhoB, T, static_cast<float*>(S));
+  else scatter_kernel<true, double><<<nb, 128, 0, st>>>(d, rhoA, rhoB, T, static_cast<double*>(S));
   return 1;
 }
-int launch_gather(const Dev& d, const double* S, double* fA, double* fB, double* g, cudaStream_t st) {
-  gather_kernel<<<blocks_for((long long)d.nx * d.ny, 128), 128, 0, st>>>(d, S, fA, fB, g);
+int launch_gather(const Dev& d, const void* S, double* fA, double* fB, double* g, cudaStream_t st) {
+  const unsigned nb = blocks_for((long long)d.nx * d.ny, 128);
+  if (d.prec == 32) gather_kernel<float><<<nb, 128, 0, st>>>(d, static_cast<const float*>(S), fA, fB, g);
+  else gather_kernel<double><<<nb, 128, 0, st>>>(d, static_cast<const double*>(S), fA, fB, g);
   return 1;
 }
-int launch_copy_g(const Dev& d, const double* Ssrc, double* Sdst, cudaStream_t st) {
-  copy_g_kernel<<<blocks_for(9ll * d.px * (d.ny + 2), 256), 256, 0, st>>>(d, Ssrc, Sdst);
+int launch_copy_g(const Dev& d, const void* Ssrc, void* Sdst, cudaStream_t st) {
+  const unsigned nb = blocks_for(9ll * d.px * (d.ny + 2), 256);
+  if (d.prec == 32) copy_g_kernel<float><<<nb, 256, 0, st>>>(d, static_cast<const float*>(Ssrc), static_cast<float*>(Sdst));
+  else copy_g_kernel<double><<<nb, 256, 0, st>>>(d, static_cast<const double*>(Ssrc), static_cast<double*>(Sdst));
   return 1;
 }
 int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st) {

@@ -47,8 +47,9 @@ struct Dev {
   int nx, ny;
   int px;                // padded row pitch in doubles (and in bytes of the padded mask)
   int periodic_y, thermal;
-  long long plane;       // doubles between consecutive planes of one node
-  long long row;         // doubles between consecutive rows of one plane
+  int prec;              // storage precision of the populations: 64 (double) or 32 (float; arithmetic stays fp64)
+  long long plane;       // elements between consecutive planes of one node
+  long long row;         // elements between consecutive rows of one plane
   double omega, omega_g; // 1/tau, 1/tau_g
   double tau;
   double inv_rho0, rho0;
@@ -68,16 +69,16 @@ __host__ __device__ inline int padded_pitch(int nx) {
 }
 
 // launchers (each returns the number of kernels it launched)
-int launch_step(const Dev& d, const double* Sin, double* Sout, int seg_rows, cudaStream_t st);
-int launch_fields(const Dev& d, const double* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
+int launch_step(const Dev& d, const void* Sin, void* Sout, int seg_rows, cudaStream_t st);
+int launch_fields(const Dev& d, const void* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
                   cudaStream_t st);
-int launch_boundary(const Dev& d, double* S, const int* sites, int n_sites, cudaStream_t st);
+int launch_boundary(const Dev& d, void* S, const int* sites, int n_sites, cudaStream_t st);
 int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st);
-int launch_scatter(const Dev& d, const double* fA, const double* fB, const double* g, double* S, cudaStream_t st);
-int launch_gather(const Dev& d, const double* S, double* fA, double* fB, double* g, cudaStream_t st);
-int launch_set_fields(const Dev& d, const double* rhoA, const double* rhoB, const double* T, double* S,
+int launch_scatter(const Dev& d, const double* fA, const double* fB, const double* g, void* S, cudaStream_t st);
+int launch_gather(const Dev& d, const void* S, double* fA, double* fB, double* g, cudaStream_t st);
+int launch_set_fields(const Dev& d, const double* rhoA, const double* rhoB, const double* T, void* S,
                       cudaStream_t st);
-int launch_copy_g(const Dev& d, const double* Ssrc, double* Sdst, cudaStream_t st);
+int launch_copy_g(const Dev& d, const void* Ssrc, void* Sdst, cudaStream_t st);
 int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* centres, int n_centres,
                 uint8_t* inside_scratch, uint8_t* solid, double* rhoA, double* rhoB, double* T, cudaStream_t st);
 int launch_observables(const Dev& d, const double* rhoA, const double* rhoB, const double* ux, const double* uy,

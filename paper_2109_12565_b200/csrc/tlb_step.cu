@@ -78,8 +78,16 @@ __device__ __forceinline__ double ldg_stream(const double* a, uint64_t policy) {
   asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(policy));
   return v;
 }
+__device__ __forceinline__ double ldg_stream(const float* a, uint64_t policy) {
+  float v;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(a), "l"(policy));
+  return (double)v;
+}
 __device__ __forceinline__ void stg_stream(double* a, double v, uint64_t policy) {
   asm volatile("st.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(a), "d"(v), "l"(policy) : "memory");
+}
+__device__ __forceinline__ void stg_stream(float* a, double v, uint64_t policy) {
+  asm volatile("st.global.L2::cache_hint.f32 [%0], %1, %2;" ::"l"(a), "f"((float)v), "l"(policy) : "memory");
 }
 
 // e^x for x <= 0 (the argument of Eq. (12) is -rho / rho0): Cody-Waite reduction x = k ln2 + r,
@@ -131,8 +139,15 @@ constexpr int kWarps = kThreads / 32;  // 8
 constexpr int kWC = 16;                // lattice columns per warp
 constexpr int kWR = kWC + 4;           // ring columns per warp: its 16 columns and a 2-cell halo each side
 
+// ST = storage type of the populations (double, or float for the pop_precision = 32 bandwidth study; the
+// arithmetic is fp64 either way).  Row stride of the landed rows in shared memory: kCopyW doubles, or
+// kCopyW + 8 floats so that the two species of a lane pair fall into disjoint banks.
+template <typename ST> struct SlotW { static constexpr int v = kCopyW; };
+template <> struct SlotW<float> { static constexpr int v = kCopyW + 8; };
+
+template <typename ST>
 struct Smem {
-  double f[kSlots][18][kCopyW];              // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
+  ST f[kSlots][18][SlotW<ST>::v];            // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
   double rho[kWarps][kRingRows][kWR][2];     // per warp: {rho_A, rho_B} per column (a lane pair reads 16 contiguous bytes,
   double psi[kWarps][kRingRows][kWR][2];     //           {psi^s_A, psi^s_B}          a half-warp 128: conflict-free)
   uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
@@ -162,13 +177,14 @@ __device__ __forceinline__ double relax(double f, double owd, double cu, double 
 // (phase 1), its force, shifted velocity, collision and 9 stores (phase 2) -- and half of the thermal
 // set: s = 0 takes g_0, g_1, g_2, g_5, g_6, s = 1 the opposite directions g_3, g_4, g_7, g_8, so both
 // lanes run the same code on (c_i, u) and (-c_i, -u).  Partial sums (j, F, T) cross by one shuffle.
-template <int MODE, bool PERIODIC>
+template <int MODE, bool PERIODIC, typename ST>
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
-fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ Sout, int seg_rows,
+fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int seg_rows,
              double* __restrict__ oRA, double* __restrict__ oRB, double* __restrict__ oUx, double* __restrict__ oUy,
              double* __restrict__ oT) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
+  Smem<ST>& sm = *reinterpret_cast<Smem<ST>*>(smem_raw);
+  constexpr int kSW = SlotW<ST>::v, kB = (int)sizeof(ST);
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const int k = lane >> 1, s = lane & 1;
@@ -179,7 +195,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   const int y0 = blockIdx.y * seg_rows;
   const int y1 = min(ny, y0 + seg_rows);
   const long long plane = d.plane;
-  const long long planeB = plane * 8, rowB = d.row * 8;
+  const long long planeB = plane * kB, rowB = d.row * kB;
   const uint64_t pol = policy_evict_first();  // every line of Sin is dead once read, Sout until the next step
 
   if (t == 0) {
@@ -203,14 +219,14 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       if (rp >= ny) rp = 0;
     }
     uint64_t* bar = &sm.full[q & 3];
-    mbar_expect_tx(bar, 18u * kCopyW * 8u);
+    mbar_expect_tx(bar, 18u * kCopyW * kB);
     const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
 #pragma unroll
     for (int l = 0; l < 2; l++)
 #pragma unroll
       for (int i = 0; i < 9; i++) {
         const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-        bulk_g2s(&sm.f[q & 3][l * 9 + i][0], Sin + (l * 9 + i) * plane + o, kCopyW * 8u, bar, pol);
+        bulk_g2s(&sm.f[q & 3][l * 9 + i][0], Sin + (l * 9 + i) * plane + o, kCopyW * kB, bar, pol);
       }
   };
   // elected lane: start the HBM -> L2 read of all 27 source plane rows of target row r
@@ -229,7 +245,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     for (int p = 0; p < 27; p++) {
       const int i = p % 9;
       const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-      if (p < np) prefetch_l2(Sin + p * plane + o, kCopyW * 8u);
+      if (p < np) prefetch_l2(Sin + p * plane + o, kCopyW * kB);
     }
   };
   if (t == 0) {
@@ -263,7 +279,7 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
   const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + d.at(x, y0));   // g_{i + 2s}
   char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + d.at(x, y0));                    // own species
   char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + d.at(x, y0));             // own thermal half
-  const int co = s ? 8 : -8;                                                                    // x - c_x of c_1 / c_3
+  const int co = s ? kB : -kB;                                                                    // x - c_x of c_1 / c_3
 
   // thermal populations of (x, y).  Lane s = 0 reads
   // g_0, g_1, g_2, g_5, g_6 at x - c_i; lane s = 1 the opposite directions at x + c_i.
@@ -274,11 +290,11 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       if (!s && y == 0) rofs = (long long)(ny - 1) * rowB;
       if (s && y == ny - 1) rofs = -(long long)(ny - 1) * rowB;
     }
-    g0 = ldg_stream(reinterpret_cast<const double*>(gp - (s ? 2 * planeB : 0)), pol);
-    ga = ldg_stream(reinterpret_cast<const double*>(gp + 1 * planeB + co), pol);
-    gb = ldg_stream(reinterpret_cast<const double*>(gp + 2 * planeB + rofs), pol);
-    gc = ldg_stream(reinterpret_cast<const double*>(gp + 5 * planeB + rofs + co), pol);
-    gd = ldg_stream(reinterpret_cast<const double*>(gp + 6 * planeB + rofs - co), pol);
+    g0 = ldg_stream(reinterpret_cast<const ST*>(gp - (s ? 2 * planeB : 0)), pol);
+    ga = ldg_stream(reinterpret_cast<const ST*>(gp + 1 * planeB + co), pol);
+    gb = ldg_stream(reinterpret_cast<const ST*>(gp + 2 * planeB + rofs), pol);
+    gc = ldg_stream(reinterpret_cast<const ST*>(gp + 5 * planeB + rofs + co), pol);
+    gd = ldg_stream(reinterpret_cast<const ST*>(gp + 6 * planeB + rofs - co), pol);
   };
 
   uint32_t parity = 0;  // one bit per slot
@@ -306,10 +322,10 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       const uint8_t sol = pass == 0 ? s0 : s1;
       double rl = rho_wall, pl = pss_wall;
       if (!sol) {
-        const double* fs = &sm.f[slot][9 * s][kWC * wid + c + 2];  // S(x) of ring column c
+        const ST* fs = &sm.f[slot][9 * s][kWC * wid + c + 2];  // S(x) of ring column c
         double f[9];
 #pragma unroll
-        for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
+        for (int i = 0; i < 9; i++) f[i] = (double)fs[i * kSW - cx(i)];
         rl = sum9(f);
         pl = d.rho0 * (1.0 - exp_nonpos(-rl * d.inv_rho0));
       }
@@ -321,9 +337,9 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
     const int slot2 = (q + 2) & 3;  // == (q - 2) & 3
     double f[9];
     {
-      const double* fs = &sm.f[slot2][9 * s][kWC * wid + k + kHX];
+      const ST* fs = &sm.f[slot2][9 * s][kWC * wid + k + kHX];
 #pragma unroll
-      for (int i = 0; i < 9; i++) f[i] = fs[i * kCopyW - cx(i)];
+      for (int i = 0; i < 9; i++) f[i] = (double)fs[i * kSW - cx(i)];
     }
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
     if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1) {  // last warp out: the slot is free
@@ -424,26 +440,26 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
       }
       if (fluid) {
 #pragma unroll
-        for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<double*>(opf + i * planeB), f[i], pol);
+        for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<ST*>(opf + i * planeB), f[i], pol);
         if (d.thermal) {
-          if (!s) stg_stream(reinterpret_cast<double*>(opg), g0, pol);
-          stg_stream(reinterpret_cast<double*>(opg + 1 * planeB), ga, pol);
-          stg_stream(reinterpret_cast<double*>(opg + 2 * planeB), gb, pol);
-          stg_stream(reinterpret_cast<double*>(opg + 5 * planeB), gc, pol);
-          stg_stream(reinterpret_cast<double*>(opg + 6 * planeB), gd, pol);
+          if (!s) stg_stream(reinterpret_cast<ST*>(opg), g0, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 1 * planeB), ga, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 2 * planeB), gb, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 5 * planeB), gc, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 6 * planeB), gd, pol);
         }
         if (x < kGhost || x >= nx - kGhost) {  // periodic images of this column (ghost columns)
           for (int pass = 0; pass < 2; pass++)
             for (int xg = pass ? x - nx : x + nx; pass ? xg >= -kGhost : xg < nx + kGhost; xg += pass ? -nx : nx) {
-              const long long e = (long long)(xg - x) * 8;
+              const long long e = (long long)(xg - x) * kB;
 #pragma unroll
-              for (int i = 0; i < 9; i++) *reinterpret_cast<double*>(opf + i * planeB + e) = f[i];
+              for (int i = 0; i < 9; i++) *reinterpret_cast<ST*>(opf + i * planeB + e) = (ST)f[i];
               if (d.thermal) {
-                if (!s) *reinterpret_cast<double*>(opg + e) = g0;
-                *reinterpret_cast<double*>(opg + 1 * planeB + e) = ga;
-                *reinterpret_cast<double*>(opg + 2 * planeB + e) = gb;
-                *reinterpret_cast<double*>(opg + 5 * planeB + e) = gc;
-                *reinterpret_cast<double*>(opg + 6 * planeB + e) = gd;
+                if (!s) *reinterpret_cast<ST*>(opg + e) = (ST)g0;
+                *reinterpret_cast<ST*>(opg + 1 * planeB + e) = (ST)ga;
+                *reinterpret_cast<ST*>(opg + 2 * planeB + e) = (ST)gb;
+                *reinterpret_cast<ST*>(opg + 5 * planeB + e) = (ST)gc;
+                *reinterpret_cast<ST*>(opg + 6 * planeB + e) = (ST)gd;
               }
             }
         }
@@ -462,8 +478,9 @@ fused_kernel(const Dev d, const double* __restrict__ Sin, double* __restrict__ S
 // x = s + c_i fluid:
 //   f:  S_i(s) = S_opp(i)(x)                         half-way bounce-back, L151 (R7)
 //   g:  S_i(s) = -S_opp(i)(x) + 2 w_i T_w(s)         fixed wall temperature, L314 (R8)
+template <typename ST>
 __global__ void __launch_bounds__(256)
-boundary_kernel(const Dev d, double* __restrict__ S, const int* __restrict__ sites, int n_sites) {
+boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, int n_sites) {
   const int nx = d.nx, ny = d.ny;
   const int n_ghost = d.periodic_y ? 0 : 2 * nx;
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -487,8 +504,8 @@ boundary_kernel(const Dev d, double* __restrict__ S, const int* __restrict__ sit
   const long long plane = d.plane;
   const long long os = d.at(sx, sy), ox = d.at(x, y);
   const int io = opp(i);
-  const double va = S[io * plane + ox], vb = S[(9 + io) * plane + ox];
-  const double vg = d.thermal ? -S[(18 + io) * plane + ox] + 2.0 * wq(i) * Tw : 0.0;
+  const ST va = S[io * plane + ox], vb = S[(9 + io) * plane + ox];
+  const ST vg = d.thermal ? (ST)(-(double)S[(18 + io) * plane + ox] + 2.0 * wq(i) * Tw) : (ST)0;
   for (int xg = sx; xg < nx + kGhost; xg += nx) {  // the node and its right-hand images
     S[i * plane + os + (xg - sx)] = va;
     S[(9 + i) * plane + os + (xg - sx)] = vb;
@@ -505,12 +522,19 @@ static dim3 strip_grid(const Dev& d, int seg_rows) {
   return dim3((d.nx + kW - 1) / kW, (d.ny + seg_rows - 1) / seg_rows);
 }
 
+template <typename ST>
+static cudaError_t configure_for() {
+  const int bytes = (int)sizeof(Smem<ST>);
+  cudaError_t e = cudaFuncSetAttribute(fused_kernel<0, false, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<0, true, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, false, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, true, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  return e;
+}
+
 int configure_kernels() {
-  const int bytes = (int)sizeof(Smem);
-  cudaError_t e = cudaFuncSetAttribute(fused_kernel<0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaError_t e = configure_for<double>();
+  if (e == cudaSuccess) e = configure_for<float>();
   return e == cudaSuccess ? 0 : (int)e;
 }
 
@@ -541,30 +565,42 @@ int default_seg_rows(int nx, int ny) {
   return best_seg;
 }
 
-int launch_step(const Dev& d, const double* Sin, double* Sout, int seg_rows, cudaStream_t st) {
-  if (d.periodic_y)
-    fused_kernel<0, true><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, Sin, Sout, seg_rows, nullptr, nullptr,
-                                                                                 nullptr, nullptr, nullptr);
-  else
-    fused_kernel<0, false><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, Sin, Sout, seg_rows, nullptr, nullptr,
-                                                                                  nullptr, nullptr, nullptr);
+template <typename ST>
+static void launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, double* rhoA, double* rhoB,
+                         double* ux, double* uy, double* T, cudaStream_t st) {
+  const ST* in = static_cast<const ST*>(Sin);
+  ST* out = static_cast<ST*>(Sout);
+  const dim3 g = strip_grid(d, seg_rows);
+  const size_t sm = sizeof(Smem<ST>);
+  if (mode == 0) {
+    if (d.periodic_y) fused_kernel<0, true, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
+    else fused_kernel<0, false, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
+  } else {
+    if (d.periodic_y) fused_kernel<1, true, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
+    else fused_kernel<1, false, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
+  }
+}
+
+int launch_step(const Dev& d, const void* Sin, void* Sout, int seg_rows, cudaStream_t st) {
+  if (d.prec == 32) launch_fused<float>(d, 0, Sin, Sout, seg_rows, nullptr, nullptr, nullptr, nullptr, nullptr, st);
+  else launch_fused<double>(d, 0, Sin, Sout, seg_rows, nullptr, nullptr, nullptr, nullptr, nullptr, st);
   return 1;
 }
 
-int launch_fields(const Dev& d, const double* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
+int launch_fields(const Dev& d, const void* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
                   cudaStream_t st) {
   const int seg_rows = default_seg_rows(d.nx, d.ny);
-  if (d.periodic_y)
-    fused_kernel<1, true><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T);
-  else
-    fused_kernel<1, false><<<strip_grid(d, seg_rows), kThreads, sizeof(Smem), st>>>(d, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T);
+  if (d.prec == 32) launch_fused<float>(d, 1, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T, st);
+  else launch_fused<double>(d, 1, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T, st);
   return 1;
 }
 
-int launch_boundary(const Dev& d, double* S, const int* sites, int n_sites, cudaStream_t st) {
+int launch_boundary(const Dev& d, void* S, const int* sites, int n_sites, cudaStream_t st) {
   const long long n = 8ll * ((d.periodic_y ? 0 : 2 * d.nx) + n_sites);
   if (n == 0) return 0;
-  boundary_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d, S, sites, n_sites);
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  if (d.prec == 32) boundary_kernel<float><<<blocks, 256, 0, st>>>(d, static_cast<float*>(S), sites, n_sites);
+  else boundary_kernel<double><<<blocks, 256, 0, st>>>(d, static_cast<double*>(S), sites, n_sites);
   return 1;
 }
 

@@ -63,9 +63,12 @@ def test_workspace_bytes_and_validation(binding):
     pops = 2 * 27 * 4096 * 2050 * 8
     assert pops < n.value < pops * 1.12  # two population buffers dominate
     for bad in (dict(tau=0.5), dict(tau_g=0.3), dict(rho0=0.0), dict(post_w=4, post_h=4, post_period=16, periodic_y=1),
-                dict(post_w=4, post_h=1024, post_period=16), dict(pop_precision=32), dict(n_droplets=-1)):
+                dict(post_w=4, post_h=1024, post_period=16), dict(pop_precision=16), dict(n_droplets=-1)):
         q = binding.default_params(**bad)
         assert lib.tlb_workspace_bytes(4096, 2048, ctypes.byref(q), ctypes.byref(n)) == binding.TLB_EINVAL, bad
+    q = binding.default_params(pop_precision=32)  # fp32 population storage: half-size buffers + a host staging area
+    m = ctypes.c_size_t()
+    assert lib.tlb_workspace_bytes(4096, 2048, ctypes.byref(q), ctypes.byref(m)) == 0 and m.value < n.value
     assert lib.tlb_workspace_bytes(0, 8, ctypes.byref(p), ctypes.byref(n)) == binding.TLB_EINVAL
     assert lib.tlb_workspace_bytes(8, 8, None, ctypes.byref(n)) == binding.TLB_EINVAL
     assert b"fallback" in lib.tlb_error_string(binding.TLB_ECUDA)

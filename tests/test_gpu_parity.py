@@ -294,3 +294,36 @@ def test_table_b8b_on_the_gpu(tlbmod):
         if g_run >= 0.45 or g_run <= 0.10:
             assert abs(rA.max() / rmax - 1) < 2e-6 and abs(rA.min() / rmin - 1) < 2e-6, (g_print, rA.max(), rA.min())
         t.close()
+
+
+def test_fp32_population_storage_study(tlbmod, oracle_mod):
+    """pop_precision = 32 (BASELINE config 5's bandwidth study): populations are stored in HBM as float, the
+    arithmetic stays fp64.  It is NOT expected to meet the 1e-12 parity bar: every stored value is rounded to
+    2^-24 relative each step.  Checked: the error against the fp64 oracle after 10 steps is of that size
+    (and nowhere near the fp64 path's 1e-15), the state stays finite, mass drifts by rounding only, and the
+    set / get round trip is exact for float-representable populations."""
+    cfg = inputs.config(1)
+    solid, rA, rB, T = inputs.make_config_inputs(dict(cfg, posts=(4, 4, 16)))
+    o = oracle_mod.Oracle(cfg["nx"], cfg["ny"], **cfg["params"])
+    t = tlbmod.TLB(cfg["nx"], cfg["ny"], **dict(cfg["params"], pop_precision=32))
+    o.set_solid(solid)
+    t.set_solid(solid)
+    o.set_fields(rA, rB, T)
+    t.set_fields(rA, rB, T)
+    m0 = t.observables()
+    o.step(10)
+    t.step(10)
+    err = _maxdiff(o, t)
+    assert 1e-10 < err < 2e-6, err
+    m1 = t.observables()
+    assert abs(m1["mass_A"] / m0["mass_A"] - 1) < 1e-6 and np.isfinite(m1["Nu"])
+    pf = [np.asarray(p, dtype=np.float32).astype(np.float64) for p in o.get_populations()]
+    t.set_populations(*pf)
+    for a, b in zip(pf, t.get_populations()):
+        assert np.array_equal(a * (solid == 0), b.cpu().numpy())
+    import torch
+    th = tlbmod.TLB(cfg["nx"], cfg["ny"], **dict(cfg["params"], pop_precision=32))
+    th.set_solid_host(torch.from_numpy(solid))
+    th.set_populations_host(*[torch.from_numpy(np.ascontiguousarray(p)) for p in pf])
+    for a, b in zip(t.get_populations(), th.get_populations_host()):
+        assert np.array_equal(a.cpu().numpy(), b.numpy())
