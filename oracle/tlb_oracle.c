@@ -21,6 +21,8 @@
  *   transport coeffs   decay of a shear wave (nu) and of a T mode (kappa)     Eqs. (14), (20)
  *   forces + pressure  Laplace law on one droplet, flat-interface coexistence Eq. (9)
  *   buoyancy           barometric density gradient at rest                    Eq. (22)
+ *   moving flat walls  exact linear Couette profile between the wall velocities, exact mass
+ *                      conservation (reading R20 of L147-151, Eq. (15))
  *   posts / corners    second, independently written streaming formulation
  *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
  *                      pull of orc_step; beyond that and mass conservation the post-corner
@@ -70,6 +72,7 @@ typedef struct orc_params {
   double T_bottom, T_top, T_ref;      /* Tdown / Tup L314; footnote 3 L182    */
   double alpha_g;                     /* Eq. (22)                             */
   double body_ax;                     /* extension: uniform acceleration in x */
+  double u_wall_bottom, u_wall_top;   /* x-velocity of the flat walls, L147-151 (R20) */
   int32_t periodic_y;                 /* L147, L284-302                       */
   int32_t thermal;                    /* THERMAL, L314                        */
 } orc_params;
@@ -301,6 +304,14 @@ static void stream_pull(orc_state *s) {
         } else {
           size_t loc = PIDX(s, OPP[i], x, y);
           s->fA[q] = s->fAs[loc]; s->fB[q] = s->fBs[loc];
+          /* R20: a flat wall (ghost row beyond y = -1/2 or ny - 1/2, not a post) moving along x with
+           * velocity u_w hands the population back with the momentum of the wall,
+           * f_i = f*_opp(i) + 2 w_i rho_l (c_i . u_w) / c_s^2, c_s^2 = 1/3 (L147-151, Eq. (15)). */
+          if (!s->p.periodic_y && (sy < 0 || sy >= ny)) {
+            double uw = sy < 0 ? s->p.u_wall_bottom : s->p.u_wall_top;
+            s->fA[q] += 6.0 * W[i] * s->rhoA[IDX(s, x, y)] * (CX[i] * uw);
+            s->fB[q] += 6.0 * W[i] * s->rhoB[IDX(s, x, y)] * (CX[i] * uw);
+          }
           if (s->p.thermal) {
             int wy = s->p.periodic_y ? wrap(sy, ny) : sy;
             s->g[q] = -s->gs[loc] + 2.0 * W[i] * T_wall(s, wy);
@@ -359,6 +370,11 @@ void orc_step_push_ghost(orc_state *s, long n) {
             int ox = wrap(gx - CX[i], nx), oy = gy - CY[i];
             if (s->p.periodic_y) oy = wrap(oy, ny);
             s->fA[PIDX(s, OPP[i], ox, oy)] = PA[d]; s->fB[PIDX(s, OPP[i], ox, oy)] = PB[d];
+            if (ty < 0 || ty >= ny) { /* moving flat wall, R20: the returned direction is opp(i) */
+              double uw = ty < 0 ? s->p.u_wall_bottom : s->p.u_wall_top;
+              s->fA[PIDX(s, OPP[i], ox, oy)] += 6.0 * W[OPP[i]] * s->rhoA[IDX(s, ox, oy)] * (CX[OPP[i]] * uw);
+              s->fB[PIDX(s, OPP[i], ox, oy)] += 6.0 * W[OPP[i]] * s->rhoB[IDX(s, ox, oy)] * (CX[OPP[i]] * uw);
+            }
             if (s->p.thermal) s->g[PIDX(s, OPP[i], ox, oy)] = -PG[d] + 2.0 * W[i] * T_wall(s, ty);
           }
         }

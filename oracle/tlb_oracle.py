@@ -29,7 +29,7 @@ def build(force=False):
 class OrcParams(ctypes.Structure):
     _fields_ = [(n, ctypes.c_double) for n in (
         "tau", "tau_g", "rho0", "G12", "G11a", "G11r", "G22a", "G22r", "rho_wall_A", "rho_wall_B",
-        "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax")] + [
+        "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax", "u_wall_bottom", "u_wall_top")] + [
         ("periodic_y", ctypes.c_int32), ("thermal", ctypes.c_int32)]
 
 
@@ -83,7 +83,7 @@ class Oracle:
         p = OrcParams()
         defaults = dict(tau=1.0, tau_g=1.0, rho0=1.0, G12=0.0, G11a=0.0, G11r=0.0, G22a=0.0, G22r=0.0,
                         rho_wall_A=0.0, rho_wall_B=0.0, T_bottom=0.0, T_top=0.0, T_ref=0.0, alpha_g=0.0,
-                        body_ax=0.0, periodic_y=0, thermal=1)
+                        body_ax=0.0, u_wall_bottom=0.0, u_wall_top=0.0, periodic_y=0, thermal=1)
         for k in PARAM_KEYS:
             setattr(p, k, params.get(k, defaults[k]))
         self.params = p

@@ -316,3 +316,30 @@ def test_laplace_law(oracle_mod):
     assert dP1 > 0 and dP2 > 0 and R2 > R1 + 3
     s1, s2 = dP1 * R1, dP2 * R2
     assert abs(s1 / s2 - 1) < 0.06, (s1, s2)
+
+
+@pytest.mark.parametrize("tau", [0.8, 1.0, 1.4])
+def test_couette_moving_walls(oracle_mod, tau):
+    """Reading R20 (L147-151, Eq. (15)): flat walls moving along x.  With G = 0 the steady state is the exact
+    linear Couette profile u_x(y) = U_b + (U_t - U_b)(y + 1/2)/ny between walls at y = -1/2 and ny - 1/2 (the
+    half-way planes of the bounce-back), for every tau; u_y = 0; each component's mass is conserved exactly
+    (the +-c_x corrections of a wall node cancel)."""
+    nx, ny, Ub, Ut = 12, 16, -0.01, 0.03
+    o = oracle_mod.Oracle(nx, ny, tau=tau, thermal=0, u_wall_bottom=Ub, u_wall_top=Ut)
+    f = np.full((ny, nx), 0.5)
+    o.set_fields(f, 1.4 * f, 0 * f)
+    m0 = _mass(o)
+    o.step(int(40 * ny * ny / ((tau - 0.5) / 3.0) / 10))
+    _, _, u, _ = o.fields()
+    expect = Ub + (Ut - Ub) * (np.arange(ny) + 0.5) / ny
+    assert np.abs(u[0] - expect[:, None]).max() < 1e-9
+    assert np.abs(u[1]).max() < 1e-12
+    m1 = _mass(o)
+    assert abs(m1[0] / m0[0] - 1) < 1e-12 and abs(m1[1] / m0[1] - 1) < 1e-12
+    # the two streaming formulations agree with moving walls too
+    o2 = oracle_mod.Oracle(nx, ny, tau=tau, thermal=0, u_wall_bottom=Ub, u_wall_top=Ut)
+    o2.set_populations(*o.get_populations())
+    o.step(3)
+    o2.step_push_ghost(3)
+    for a, b in zip(o.get_populations(), o2.get_populations()):
+        assert np.array_equal(a, b)
