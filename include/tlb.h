@@ -63,6 +63,7 @@ typedef struct tlb_params {
   double T_bottom, T_top, T_ref;      /* wall temperatures L314; buoyancy reference, footnote L182 (R12)    */
   double alpha_g;                     /* alpha*g of Eq. (22)                                                */
   double body_ax;                     /* EXTENSION: uniform acceleration along x (Poiseuille test)          */
+  double u_wall_bottom, u_wall_top;   /* x-velocity of the flat walls (Couette, L147-151, Eq. (15); R20)    */
   /* input recipe used by tlb_init only */
   double droplet_radius, min_gap, rho_in, rho_out, noise_amp;
   int32_t n_droplets;
@@ -87,7 +88,7 @@ int tlb_workspace_bytes(int nx, int ny, const tlb_params* p, size_t* bytes);
 
 /* Create a handle on `workspace` (DEVICE pointer, >= tlb_workspace_bytes, 256-byte aligned, caller
  * owned) that enqueues all work on `stream` (a cudaStream_t passed as void*; NULL = default stream).
- * TLB_EINVAL: nx, ny < 1, tau or tau_g <= 1/2, rho0 <= 0, posts with periodic_y (the paper's own
+ * TLB_EINVAL: nx, ny < 1, tau or tau_g <= 1/2, rho0 <= 0, moving walls or posts with periodic_y (the paper's own
  * warning, footnote L302), 2*post_h >= ny, post_w > post_period, NULL pointers, workspace too small. */
 int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t workspace_bytes,
                void* stream, tlb_handle** out);

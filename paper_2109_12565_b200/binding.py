@@ -31,7 +31,7 @@ class TLBParams(ctypes.Structure):
     """Mirror of `struct tlb_params` (include/tlb.h)."""
     _fields_ = [(n, ctypes.c_double) for n in (
         "tau", "tau_g", "rho0", "G12", "G11a", "G11r", "G22a", "G22r", "rho_wall_A", "rho_wall_B",
-        "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax",
+        "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax", "u_wall_bottom", "u_wall_top",
         "droplet_radius", "min_gap", "rho_in", "rho_out", "noise_amp")] + [(n, ctypes.c_int32) for n in (
             "n_droplets", "periodic_y", "thermal", "post_w", "post_h", "post_period", "pop_precision", "reserved")]
 

@@ -75,6 +75,7 @@ bool params_ok(int nx, int ny, const tlb_params* p) {
   if (p->n_droplets < 0 || p->post_w < 0 || p->post_h < 0 || p->post_period < 0) return false;
   const bool posts = p->post_w > 0 && p->post_h > 0 && p->post_period > 0;
   if (posts && (p->periodic_y || 2 * p->post_h >= ny || p->post_w > p->post_period)) return false;
+  if (p->periodic_y && (p->u_wall_bottom != 0.0 || p->u_wall_top != 0.0)) return false;  // no walls to move
   return true;
 }
 
@@ -270,6 +271,7 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   d.pss_wall_A = p->rho0 * (1.0 - std::exp(-p->rho_wall_A / p->rho0));  // Eq. (12) at the wall density
   d.pss_wall_B = p->rho0 * (1.0 - std::exp(-p->rho_wall_B / p->rho0));
   d.T_bottom = p->T_bottom; d.T_top = p->T_top; d.T_ref = p->T_ref; d.alpha_g = p->alpha_g; d.body_ax = p->body_ax;
+  d.u_wall_bottom = p->u_wall_bottom; d.u_wall_top = p->u_wall_top;
   d.solid = h->solid;
   d.solidp = h->solidp;
   h->cur = 0; h->n_sites = 0; h->has_state = false; h->err = cudaSuccess; h->launches = 0;

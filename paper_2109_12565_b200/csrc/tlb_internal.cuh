@@ -56,6 +56,7 @@ struct Dev {
   double G12, G11a, G11r, G22a, G22r;
   double rho_wall_A, rho_wall_B, pss_wall_A, pss_wall_B; // wall densities and their psi^s (Eq. 12)
   double T_bottom, T_top, T_ref, alpha_g, body_ax;
+  double u_wall_bottom, u_wall_top;  // x-velocity of the flat walls (R20)
   const uint8_t* solid;  // [ny][nx]   flag field in the API layout (L286)
   const uint8_t* solidp; // [ny][px]   the same with ghost columns, lattice column x at kXL + x
 

@@ -504,7 +504,17 @@ boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, 
   const long long plane = d.plane;
   const long long os = d.at(sx, sy), ox = d.at(x, y);
   const int io = opp(i);
-  const ST va = S[io * plane + ox], vb = S[(9 + io) * plane + ox];
+  ST va = S[io * plane + ox], vb = S[(9 + io) * plane + ox];
+  // R20: a moving flat wall (ghost row, not a post) hands the population back with the wall's momentum,
+  // f_i = f*_opp(i) + 2 w_i rho_l (c_i . u_w) / c_s^2; rho_l(x) = sum_j S_l,j(x) (collision conserves it)
+  const double uw = sy < 0 ? d.u_wall_bottom : (sy >= ny ? d.u_wall_top : 0.0);
+  if (uw != 0.0 && cx(i) != 0) {
+    double ra = 0.0, rb = 0.0;
+#pragma unroll
+    for (int j = 0; j < 9; j++) { ra += (double)S[j * plane + ox]; rb += (double)S[(9 + j) * plane + ox]; }
+    va = (ST)((double)va + 6.0 * wq(i) * ra * (cx(i) * uw));
+    vb = (ST)((double)vb + 6.0 * wq(i) * rb * (cx(i) * uw));
+  }
   const ST vg = d.thermal ? (ST)(-(double)S[(18 + io) * plane + ox] + 2.0 * wq(i) * Tw) : (ST)0;
   for (int xg = sx; xg < nx + kGhost; xg += nx) {  // the node and its right-hand images
     S[i * plane + os + (xg - sx)] = va;

@@ -37,10 +37,10 @@ def uniform(seed, stream, k):
 # physics of BASELINE.json's configs ("literal" set) and of the paper's Table A.3 ("paper" set)
 LITERAL_PHYSICS = dict(tau=1.0, tau_g=1.0, rho0=1.0, G12=0.405, G11a=-9.0, G11r=8.1, G22a=-9.0, G22r=8.1,
                        rho_wall_A=0.52, rho_wall_B=0.52, T_bottom=1.0, T_top=0.0, T_ref=0.5, alpha_g=1e-4,
-                       body_ax=0.0, periodic_y=0, thermal=1)
+                       body_ax=0.0, u_wall_bottom=0.0, u_wall_top=0.0, periodic_y=0, thermal=1)
 PAPER_PHYSICS = dict(tau=1.0, tau_g=1.0, rho0=0.83, G12=0.405, G11a=-9.0, G11r=8.1, G22a=-8.0, G22r=7.1,
                      rho_wall_A=0.612, rho_wall_B=0.612, T_bottom=0.5, T_top=-0.5, T_ref=0.0, alpha_g=1.24e-5,
-                     body_ax=0.0, periodic_y=0, thermal=1)
+                     body_ax=0.0, u_wall_bottom=0.0, u_wall_top=0.0, periodic_y=0, thermal=1)
 
 
 def config(index, physics="literal"):

@@ -47,7 +47,7 @@ def test_library_is_sm100a_and_product_never_imports_oracle(binding):
 
 
 def test_params_struct_and_defaults(binding):
-    assert ctypes.sizeof(binding.TLBParams) == 20 * 8 + 8 * 4
+    assert ctypes.sizeof(binding.TLBParams) == 22 * 8 + 8 * 4
     p = binding.default_params()
     assert (p.tau, p.tau_g, p.rho0, p.G12, p.G11a, p.G11r) == (1.0, 1.0, 1.0, 0.405, -9.0, 8.1)
     assert (p.T_bottom, p.T_top, p.T_ref, p.alpha_g, p.thermal, p.periodic_y) == (1.0, 0.0, 0.5, 1e-4, 1, 0)

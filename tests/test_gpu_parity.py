@@ -327,3 +327,34 @@ def test_fp32_population_storage_study(tlbmod, oracle_mod):
     th.set_populations_host(*[torch.from_numpy(np.ascontiguousarray(p)) for p in pf])
     for a, b in zip(t.get_populations(), th.get_populations_host()):
         assert np.array_equal(a.cpu().numpy(), b.numpy())
+
+
+def test_moving_walls_couette(tlbmod, oracle_mod):
+    """Reading R20 (L147-151, Eq. (15)): flat walls moving along x.  Parity with the oracle on a two-component
+    state with posts on the moving walls, then the exact linear Couette profile through the CUDA path."""
+    nx, ny = 200, 40
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-5, u_wall_bottom=-0.02, u_wall_top=0.03)
+    solid = inputs.post_mask(nx, ny, 3, 3, 12)
+    o, t = _pair(tlbmod, oracle_mod, nx, ny, par, solid)
+    rA, rB, T = inputs.smooth_random_fields(nx, ny, 13, 0.5, -0.5)
+    o.set_fields(rA, rB, T)
+    t.set_fields(rA, rB, T)
+    o.step(10)
+    t.step(10)
+    assert _maxdiff(o, t) <= TOL
+    _check_fields(o, t)
+    # single-phase Couette: steady state is the linear profile between the wall velocities
+    nx, ny, Ub, Ut = 12, 16, -0.01, 0.03
+    t = tlbmod.TLB(nx, ny, tau=0.8, thermal=0, G12=0.0, G11a=0.0, G11r=0.0, G22a=0.0, G22r=0.0, alpha_g=0.0,
+                   u_wall_bottom=Ub, u_wall_top=Ut)
+    f = np.full((ny, nx), 0.5)
+    t.set_fields(f, 1.4 * f, 0 * f)
+    m0 = t.observables()
+    t.step(10240)
+    u = t.fields()[2].cpu().numpy()
+    expect = Ub + (Ut - Ub) * (np.arange(ny) + 0.5) / ny
+    assert np.abs(u[0] - expect[:, None]).max() < 1e-9 and np.abs(u[1]).max() < 1e-12
+    m1 = t.observables()
+    assert abs(m1["mass_A"] / m0["mass_A"] - 1) < 1e-12
+    with pytest.raises(tlbmod.TLBError):
+        tlbmod.TLB(16, 16, periodic_y=1, u_wall_top=0.01)
