@@ -138,6 +138,12 @@ int tlb_fields_host(tlb_handle* h, double* rho_A, double* rho_B, double* u, doub
 int tlb_observables(tlb_handle* h, double* out4);
 int tlb_observables_host(tlb_handle* h, double* out4);
 
+/* u_av[ny] (DEVICE pointer; _host: HOST pointer, synchronises): the x-average over the fluid sites of every
+ * row of u_x^(H), the profile the paper dumps as u_av.dat for the Couette rheology (L248-250, Eq. (23));
+ * 0 for a row without fluid sites.  Deterministic (one CTA per row, fixed-order sums). */
+int tlb_x_average(tlb_handle* h, double* u_av);
+int tlb_x_average_host(tlb_handle* h, double* u_av);
+
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t tlb_launch_count(const tlb_handle* h);
 

@@ -436,6 +436,19 @@ void orc_observables(orc_state *s, double out[4]) {
   out[3] = (nf && DT != 0.0) ? (double)((uT / nf - kappa * (dT / nf)) / (kappa * DT / ny)) : 0.0;
 }
 
+/* x-averaged velocity profile of the Couette output u_av: u_av[y] = mean over the fluid
+ * sites of row y of u_x^(H); 0 for a row without fluid sites. */
+void orc_x_average(orc_state *s, double *u_av) {
+  moments_and_forces(s);
+  for (int y = 0; y < s->ny; y++) {
+    long double a = 0;
+    long n = 0;
+    for (int x = 0; x < s->nx; x++)
+      if (!s->solid[IDX(s, x, y)]) { a += s->uHx[IDX(s, x, y)]; n++; }
+    u_av[y] = n ? (double)(a / n) : 0.0;
+  }
+}
+
 /* lattice constants exported for the weight-invariant pins */
 double orc_w(int dx, int dy) { return w_of_c2(dx * dx + dy * dy); }
 double orc_p(int dx, int dy) { return p_of_c2(dx * dx + dy * dy); }

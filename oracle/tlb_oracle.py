@@ -53,6 +53,7 @@ def _load():
         lib.orc_fields.argtypes = [ctypes.c_void_p, dp, dp, dp, dp]
         lib.orc_forces.argtypes = [ctypes.c_void_p, dp, dp]
         lib.orc_observables.argtypes = [ctypes.c_void_p, dp]
+        lib.orc_x_average.argtypes = [ctypes.c_void_p, dp]
         lib.orc_w.restype = ctypes.c_double
         lib.orc_w.argtypes = [ctypes.c_int, ctypes.c_int]
         lib.orc_p.restype = ctypes.c_double
@@ -137,6 +138,16 @@ class Oracle:
         out = np.empty(4)
         self.lib.orc_observables(self.h, _dp(out))
         return dict(mass_A=out[0], mass_B=out[1], E=out[2], Nu=out[3])
+
+
+def _x_average(self):
+    """u_av[y]: x-average of u_x^(H) over the fluid sites of each row."""
+    out = np.empty(self.ny)
+    self.lib.orc_x_average(self.h, _dp(out))
+    return out
+
+
+Oracle.x_average = _x_average
 
 
 def lattice_weights():

@@ -23,7 +23,8 @@ SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destr
            "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
            "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step",
            "tlb_profile_step", "tlb_fields",
-           "tlb_fields_host", "tlb_observables", "tlb_observables_host", "tlb_launch_count", "tlb_error_string",
+           "tlb_fields_host", "tlb_observables", "tlb_observables_host", "tlb_x_average", "tlb_x_average_host",
+           "tlb_launch_count", "tlb_error_string",
            "tlb_last_cuda_error"]
 
 
@@ -94,6 +95,8 @@ def load_library():
     lib.tlb_fields_host.argtypes = [vp, dp, dp, dp, dp]
     lib.tlb_observables.argtypes = [vp, dp]
     lib.tlb_observables_host.argtypes = [vp, dp]
+    lib.tlb_x_average.argtypes = [vp, dp]
+    lib.tlb_x_average_host.argtypes = [vp, dp]
     lib.tlb_launch_count.argtypes = [vp]
     lib.tlb_launch_count.restype = i64
     lib.tlb_error_string.argtypes = [i32]
@@ -250,6 +253,19 @@ class TLB:
         out = (ctypes.c_double * 4)()
         self._chk(self.lib.tlb_observables_host(self.h, ctypes.cast(out, ctypes.c_void_p)))
         return dict(mass_A=out[0], mass_B=out[1], E=out[2], Nu=out[3])
+
+    def x_average(self):
+        """u_av[ny]: x-average of u_x^(H) over the fluid sites of each row (device tensor)."""
+        out = self._new(self.ny)
+        self._chk(self.lib.tlb_x_average(self.h, out.data_ptr()))
+        return out
+
+    def x_average_host(self, out=None):
+        if out is None:
+            out = self.torch.empty(self.ny, dtype=self.torch.float64)
+        out = self._host(out, (self.ny,))
+        self._chk(self.lib.tlb_x_average_host(self.h, out.data_ptr()))
+        return out
 
     def observables_device(self, out4):
         self._chk(self.lib.tlb_observables(self.h, out4.data_ptr()))

@@ -491,6 +491,25 @@ int tlb_observables_host(tlb_handle* h, double* out4) {
   return check(h);
 }
 
+int tlb_x_average(tlb_handle* h, double* u_av) {
+  if (!h || !u_av) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  fields_to_scratch(h);
+  h->launches += launch_x_average(h->d, h->fld[2], u_av, h->st);
+  return check(h);
+}
+
+int tlb_x_average_host(tlb_handle* h, double* u_av) {
+  if (!h || !u_av) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  fields_to_scratch(h);
+  // fld[0] (rho_A scratch) is free once the profile has been reduced from fld[2]
+  h->launches += launch_x_average(h->d, h->fld[2], h->fld[0], h->st);
+  cu(h, cudaMemcpyAsync(u_av, h->fld[0], (size_t)h->d.ny * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
 int64_t tlb_launch_count(const tlb_handle* h) { return h ? h->launches : 0; }
 
 const char* tlb_error_string(int code) {

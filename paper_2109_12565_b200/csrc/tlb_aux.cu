@@ -225,6 +225,25 @@ __global__ void observables_final_kernel(const Dev d, const double* __restrict__
   }
 }
 
+// one CTA per row: x-average of u_x over the fluid sites (u_av of PAPER L248-250), fixed-order sums
+__global__ void __launch_bounds__(256)
+x_average_kernel(const Dev d, const double* __restrict__ ux, double* __restrict__ u_av) {
+  const int y = blockIdx.x;
+  double a = 0.0, n = 0.0;
+  for (int x = threadIdx.x; x < d.nx; x += 256)
+    if (!d.solid[(size_t)y * d.nx + x]) { a += ux[(size_t)y * d.nx + x]; n += 1.0; }
+  __shared__ double sa[8], sn[8];
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { a += __shfl_down_sync(0xffffffffu, a, o); n += __shfl_down_sync(0xffffffffu, n, o); }
+  if ((threadIdx.x & 31) == 0) { sa[threadIdx.x >> 5] = a; sn[threadIdx.x >> 5] = n; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double ta = 0.0, tn = 0.0;
+    for (int w = 0; w < 8; w++) { ta += sa[w]; tn += sn[w]; }
+    u_av[y] = tn > 0.0 ? ta / tn : 0.0;
+  }
+}
+
 inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
 }  // namespace
@@ -269,6 +288,10 @@ int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* 
   }
   init_fields_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, p, seed, inside, solid, rhoA, rhoB, T);
   return launches;
+}
+int launch_x_average(const Dev& d, const double* ux, double* u_av, cudaStream_t st) {
+  x_average_kernel<<<d.ny, 256, 0, st>>>(d, ux, u_av);
+  return 1;
 }
 int launch_observables(const Dev& d, const double* rhoA, const double* rhoB, const double* ux, const double* uy,
                        const double* T, double* partials, int n_blocks, double* out4, cudaStream_t st) {

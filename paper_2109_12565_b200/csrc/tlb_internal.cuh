@@ -84,6 +84,7 @@ int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* 
                 uint8_t* inside_scratch, uint8_t* solid, double* rhoA, double* rhoB, double* T, cudaStream_t st);
 int launch_observables(const Dev& d, const double* rhoA, const double* rhoB, const double* ux, const double* uy,
                        const double* T, double* partials, int n_blocks, double* out4, cudaStream_t st);
+int launch_x_average(const Dev& d, const double* ux, double* u_av, cudaStream_t st);
 int configure_kernels();  // opt in to the dynamic shared memory the fused kernel needs; 0 on success
 int default_seg_rows(int nx, int ny);
 constexpr int kObsBlocks = 592; // 4 per SM on 148 SMs

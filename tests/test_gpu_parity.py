@@ -343,6 +343,8 @@ def test_moving_walls_couette(tlbmod, oracle_mod):
     t.step(10)
     assert _maxdiff(o, t) <= TOL
     _check_fields(o, t)
+    assert np.abs(o.x_average() - t.x_average().cpu().numpy()).max() <= 1e-13  # u_av (L248-250), posts excluded
+    assert np.array_equal(t.x_average().cpu().numpy(), t.x_average_host().numpy())
     # single-phase Couette: steady state is the linear profile between the wall velocities
     nx, ny, Ub, Ut = 12, 16, -0.01, 0.03
     t = tlbmod.TLB(nx, ny, tau=0.8, thermal=0, G12=0.0, G11a=0.0, G11r=0.0, G22a=0.0, G22r=0.0, alpha_g=0.0,

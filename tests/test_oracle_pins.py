@@ -334,6 +334,8 @@ def test_couette_moving_walls(oracle_mod, tau):
     expect = Ub + (Ut - Ub) * (np.arange(ny) + 0.5) / ny
     assert np.abs(u[0] - expect[:, None]).max() < 1e-9
     assert np.abs(u[1]).max() < 1e-12
+    assert np.abs(o.x_average() - expect).max() < 1e-9  # the u_av profile of L248-250; shear rate of Eq. (23)
+    assert abs((o.x_average()[-1] - o.x_average()[0]) / (ny - 1) - (Ut - Ub) / ny) < 1e-10
     m1 = _mass(o)
     assert abs(m1[0] / m0[0] - 1) < 1e-12 and abs(m1[1] / m0[1] - 1) < 1e-12
     # the two streaming formulations agree with moving walls too
