@@ -169,6 +169,11 @@ __device__ __forceinline__ double pair(double v) { return __shfl_xor_sync(0xffff
 __device__ __forceinline__ double relax(double f, double owd, double cu, double usq, double om1) {
   return om1 * f + owd * (usq + 3.0 * cu + 4.5 * cu * cu);
 }
+// the same for tau = 1 (omega = 1, every BASELINE config): the population relaxes onto its equilibrium and
+// (1 - omega) f = 0 exactly, so the result is bit-identical to relax() with one multiply less
+__device__ __forceinline__ double relax_tau1(double owd, double cu, double usq) {
+  return owd * (usq + 3.0 * cu + 4.5 * cu * cu);
+}
 
 }  // namespace
 
@@ -417,26 +422,46 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
         const double vx = ux + Fx * invl, vy = uy + Fy * invl;
         const double usq = 1.0 - 1.5 * (vx * vx + vy * vy);
         const double w0 = d.omega * (wq(0) * rl), w1 = d.omega * (wq(1) * rl), w5 = d.omega * (wq(5) * rl);
-        f[0] = relax(f[0], w0, 0.0, usq, om1);
-        f[1] = relax(f[1], w1, vx, usq, om1);
-        f[2] = relax(f[2], w1, vy, usq, om1);
-        f[3] = relax(f[3], w1, -vx, usq, om1);
-        f[4] = relax(f[4], w1, -vy, usq, om1);
-        f[5] = relax(f[5], w5, vx + vy, usq, om1);
-        f[6] = relax(f[6], w5, -vx + vy, usq, om1);
-        f[7] = relax(f[7], w5, -vx - vy, usq, om1);
-        f[8] = relax(f[8], w5, vx - vy, usq, om1);
+        if (om1 == 0.0) {  // uniform branch
+          f[0] = relax_tau1(w0, 0.0, usq);
+          f[1] = relax_tau1(w1, vx, usq);
+          f[2] = relax_tau1(w1, vy, usq);
+          f[3] = relax_tau1(w1, -vx, usq);
+          f[4] = relax_tau1(w1, -vy, usq);
+          f[5] = relax_tau1(w5, vx + vy, usq);
+          f[6] = relax_tau1(w5, -vx + vy, usq);
+          f[7] = relax_tau1(w5, -vx - vy, usq);
+          f[8] = relax_tau1(w5, vx - vy, usq);
+        } else {
+          f[0] = relax(f[0], w0, 0.0, usq, om1);
+          f[1] = relax(f[1], w1, vx, usq, om1);
+          f[2] = relax(f[2], w1, vy, usq, om1);
+          f[3] = relax(f[3], w1, -vx, usq, om1);
+          f[4] = relax(f[4], w1, -vy, usq, om1);
+          f[5] = relax(f[5], w5, vx + vy, usq, om1);
+          f[6] = relax(f[6], w5, -vx + vy, usq, om1);
+          f[7] = relax(f[7], w5, -vx - vy, usq, om1);
+          f[8] = relax(f[8], w5, vx - vy, usq, om1);
+        }
       }
       // own half of the thermal set: Eqs. (16), (18) with u^(H); directions sgn * {c_1, c_2, c_5, c_6}
       if (d.thermal) {
         const double vx = sgn * uHx, vy = sgn * uHy;
         const double usq = 1.0 - 1.5 * (uHx * uHx + uHy * uHy);
         const double w0 = d.omega_g * (wq(0) * T), w1 = d.omega_g * (wq(1) * T), w5 = d.omega_g * (wq(5) * T);
-        g0 = relax(g0, w0, 0.0, usq, om1g);
-        ga = relax(ga, w1, vx, usq, om1g);
-        gb = relax(gb, w1, vy, usq, om1g);
-        gc = relax(gc, w5, vx + vy, usq, om1g);
-        gd = relax(gd, w5, -vx + vy, usq, om1g);
+        if (om1g == 0.0) {  // uniform branch
+          g0 = relax_tau1(w0, 0.0, usq);
+          ga = relax_tau1(w1, vx, usq);
+          gb = relax_tau1(w1, vy, usq);
+          gc = relax_tau1(w5, vx + vy, usq);
+          gd = relax_tau1(w5, -vx + vy, usq);
+        } else {
+          g0 = relax(g0, w0, 0.0, usq, om1g);
+          ga = relax(ga, w1, vx, usq, om1g);
+          gb = relax(gb, w1, vy, usq, om1g);
+          gc = relax(gc, w5, vx + vy, usq, om1g);
+          gd = relax(gd, w5, -vx + vy, usq, om1g);
+        }
       }
       if (fluid) {
 #pragma unroll
