@@ -359,27 +359,28 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     const bool fluid = x < nx && !flag[rq0][cc];
     const double rl = rho_r[rq0][cc][s], rn = rho_r[rq0][cc][1 - s], pl = psi_r[rq0][cc][s];
     // force sums over the 5x5 neighbourhood: cross (w, other species' rho), self (G_a w + G_r p, own psi^s)
+    // The stencils are antisymmetric (the term of -c is minus the term of +c), so opposite neighbours are
+    // paired first: one subtraction serves both force components.
     double Xx = 0, Xy = 0, Sx = 0, Sy = 0, Sx2 = 0, Sy2 = 0;  // S = S + S2: two dependency chains per component
 #pragma unroll
-    for (int dy = -2; dy <= 2; dy++) {
-      const int sl = (q + kRingRows - 2 + dy) % kRingRows;
+    for (int dy = 0; dy <= 2; dy++) {
+      const int slp = (q + kRingRows - 2 + dy) % kRingRows, slm = (q + kRingRows - 2 - dy) % kRingRows;
 #pragma unroll
       for (int dx = -2; dx <= 2; dx++) {
+        if (dy == 0 && dx <= 0) continue;  // one representative of every pair {c, -c}
         const int c2 = dx * dx + dy * dy;
-        if (c2 == 0) continue;
         const double kk = c2 == 1 ? k1 : c2 == 2 ? k2 : c2 == 4 ? k4 : c2 == 5 ? k5 : k8;      // |component| = 1
         const double kd = c2 == 4 ? k4d : c2 == 5 ? k5d : k8d;                                  // |component| = 2
-        const double ns = psi_r[sl][cc + dx][s];
-        double& ax = dy > 0 ? Sx2 : Sx;
-        double& ay = dx > 0 ? Sy2 : Sy;
-        if (dx > 0) ax += (dx == 1 ? kk : kd) * ns;
-        if (dx < 0) ax -= (dx == -1 ? kk : kd) * ns;
-        if (dy > 0) ay += (dy == 1 ? kk : kd) * ns;
-        if (dy < 0) ay -= (dy == -1 ? kk : kd) * ns;
+        const double dpsi = psi_r[slp][cc + dx][s] - psi_r[slm][cc - dx][s];
+        double& ax = (dy & 1) ? Sx2 : Sx;
+        double& ay = (dx & 1) ? Sy2 : Sy;
+        if (dx > 0) ax += (dx == 1 ? kk : kd) * dpsi;
+        if (dx < 0) ax -= (dx == -1 ? kk : kd) * dpsi;
+        if (dy > 0) ay += (dy == 1 ? kk : kd) * dpsi;
         if (c2 <= 2) {
-          const double nr = rho_r[sl][cc + dx][1 - s];
-          if (dx != 0) Xx += (w_c2(c2) * dx) * nr;
-          if (dy != 0) Xy += (w_c2(c2) * dy) * nr;
+          const double drho = rho_r[slp][cc + dx][1 - s] - rho_r[slm][cc - dx][1 - s];
+          if (dx != 0) Xx += (w_c2(c2) * dx) * drho;
+          if (dy != 0) Xy += (w_c2(c2) * dy) * drho;
         }
       }
     }
