@@ -23,6 +23,9 @@
  *   buoyancy           barometric density gradient at rest                    Eq. (22)
  *   moving flat walls  exact linear Couette profile between the wall velocities, exact mass
  *                      conservation (reading R20 of L147-151, Eq. (15))
+ *   observables        mass, E and the convective term of Nu against closed forms on states with
+ *                      known moments (random masks, posts, buoyancy so that u^(H) != u);
+ *                      u_av on rows through posts                            L248, Eq. (24)
  *   posts / corners    second, independently written streaming formulation
  *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
  *                      pull of orc_step; beyond that and mass conservation the post-corner

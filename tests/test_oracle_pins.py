@@ -345,3 +345,111 @@ def test_couette_moving_walls(oracle_mod, tau):
     o2.step_push_ghost(3)
     for a, b in zip(o.get_populations(), o2.get_populations()):
         assert np.array_equal(a, b)
+
+
+# ---- pins of orc_observables / orc_x_average (a10; Eq. (24)) ----------------
+# The state is set through set_populations with populations whose moments are known in closed form:
+# f_i = w_i rho (1 + 3 c_i . U) has sum_i f_i = rho and sum_i c_i f_i = rho U exactly (sum w = 1,
+# sum w c = 0, sum w c c = 1/3, Fig. 1(b)), whatever the oracle's equilibrium looks like.  All G = 0, so the
+# only force is the buoyancy of Eq. (22) and L139 gives u^(H) = j / rho + alpha_g (T - T_ref) e_y / 2.
+_CX = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1])[:, None, None]
+_CY = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1])[:, None, None]
+_WQ = np.array([4 / 9] + [1 / 9] * 4 + [1 / 36] * 4)[:, None, None]
+
+
+def _linear_pops(dens, ux, uy):
+    return _WQ * dens * (1 + 3 * (_CX * ux + _CY * uy))
+
+
+def _flow_state(nx, ny, seed):
+    """Spatially varying densities, per-species velocities and temperature (all smooth and positive)."""
+    rA, rB, T = inputs.smooth_random_fields(nx, ny, seed, 1.0, 0.25)
+    x = np.arange(nx)[None, :] * (2 * np.pi / nx)
+    y = np.arange(ny)[:, None] * (2 * np.pi / ny)
+    UA = (0.03 + 0.01 * np.sin(x + y), -0.02 + 0.015 * np.cos(2 * x - y))
+    UB = (-0.01 + 0.02 * np.cos(x) * np.sin(y), 0.025 + 0.01 * np.sin(3 * x + y))
+    return rA, rB, T, UA, UB
+
+
+@pytest.mark.parametrize("geom", ["walls", "random_mask", "periodic_y_mask"])
+def test_observables_mass_and_energy_closed_form(oracle_mod, geom):
+    """mass_l = sum over FLUID sites of rho_l (north_star); E = (1/N_fluid) sum |u^(H)|^2 (L248, R11) with
+    u^(H) = (rho_A U_A + rho_B U_B) / (rho_A + rho_B) + alpha_g (T - T_ref) e_y / 2 (Eq. (5), Eq. (22)).
+    Catches: solid sites counted (they carry rho_wall), division by nx*ny, a dropped u_y^2, u instead of u^(H),
+    one species' momentum missing from Eq. (5)."""
+    nx, ny, ag, Tref = 24, 18, 3e-2, 0.4
+    solid = np.zeros((ny, nx), np.uint8)
+    if geom != "walls":
+        solid = (inputs.uniform(21, 9, np.arange(nx * ny)).reshape(ny, nx) < 0.15).astype(np.uint8)
+    o = oracle_mod.Oracle(nx, ny, tau=0.9, tau_g=1.3, rho0=0.83, rho_wall_A=0.612, rho_wall_B=0.37, T_bottom=1.0,
+                          T_top=0.25, T_ref=Tref, alpha_g=ag, periodic_y=1 if geom == "periodic_y_mask" else 0)
+    o.set_solid(solid)
+    rA, rB, T, UA, UB = _flow_state(nx, ny, 31)
+    fl = solid == 0
+    o.set_populations(_linear_pops(rA, *UA) * fl, _linear_pops(rB, *UB) * fl, _linear_pops(T, 0.1, -0.2) * fl)
+    ob = o.observables()
+    rho = rA + rB
+    uHx = (rA * UA[0] + rB * UB[0]) / rho
+    uHy = (rA * UA[1] + rB * UB[1]) / rho + 0.5 * ag * (T - Tref)
+    assert ob["mass_A"] == pytest.approx(rA[fl].sum(), rel=1e-13)
+    assert ob["mass_B"] == pytest.approx(rB[fl].sum(), rel=1e-13)
+    assert ob["E"] == pytest.approx((uHx ** 2 + uHy ** 2)[fl].mean(), rel=1e-12)
+    # the alternatives a plausible mistake would produce are far outside that tolerance
+    assert abs((uHx ** 2 + uHy ** 2)[fl].sum() / (nx * ny) / ob["E"] - 1) > 1e-3 or geom == "walls"
+    assert abs((uHx ** 2)[fl].mean() / ob["E"] - 1) > 1e-2
+    # fields() reports the same u^(H), rho and T
+    fA, fB, u, Tf = o.fields()
+    assert np.abs(u[0] - uHx)[fl].max() < 1e-15 and np.abs(u[1] - uHy)[fl].max() < 1e-15
+    assert np.abs(Tf - T)[fl].max() < 1e-15 and np.abs(fA - rA)[fl].max() < 1e-15
+
+
+@pytest.mark.parametrize("tau_g", [0.7, 1.0, 1.6])
+@pytest.mark.parametrize("geom", ["walls", "posts"])
+def test_nusselt_convective_term_closed_form(oracle_mod, tau_g, geom):
+    """Eq. (24) L347 in the reading R10: Nu = [<u_y^(H) T> - kappa <d_y T>] / (kappa dT / ny), kappa of Eq. (20).
+    Between walls the face differences of R10 telescope along every column to T_top - T_bottom WHATEVER the
+    interior temperature is (each column of this geometry is one fluid run from a T_bottom node to a T_top
+    node), so <d_y T> = -dT * n_columns / N_fluid and
+        Nu = [<u_y^(H) T> + kappa dT n_columns / N_fluid] * ny / (kappa dT),
+    with <u_y^(H) T> the fluid-site mean of the known velocity times the known temperature.  Catches the sign,
+    the velocity (u vs u^(H), x vs y), the normalisation (N_fluid) and kappa of the convective term, which the
+    conduction pin (u = 0) never sees."""
+    nx, ny, ag, Tref, Tb, Tt = 32, 20, 2e-2, 0.1, 1.0, 0.25
+    solid = inputs.post_mask(nx, ny, 4, 3, 8) if geom == "posts" else np.zeros((ny, nx), np.uint8)
+    o = oracle_mod.Oracle(nx, ny, tau=1.1, tau_g=tau_g, T_bottom=Tb, T_top=Tt, T_ref=Tref, alpha_g=ag)
+    o.set_solid(solid)
+    rA, rB, T, UA, UB = _flow_state(nx, ny, 32)
+    fl = solid == 0
+    o.set_populations(_linear_pops(rA, *UA) * fl, _linear_pops(rB, *UB) * fl, _linear_pops(T, -0.05, 0.07) * fl)
+    uHy = (rA * UA[1] + rB * UB[1]) / (rA + rB) + 0.5 * ag * (T - Tref)
+    kappa, dT = (tau_g - 0.5) / 3, Tb - Tt
+    expect = ((uHy * T)[fl].mean() + kappa * dT * nx / fl.sum()) * ny / (kappa * dT)
+    assert o.observables()["Nu"] == pytest.approx(expect, rel=1e-12)
+    assert abs(expect - 1) > 0.3  # the convective term matters in this state
+    # uniform rise U through a linear profile: Nu = 1 + U <T> ny / (kappa dT) (no posts, no buoyancy)
+    if geom == "walls":
+        U = 0.013
+        o2 = oracle_mod.Oracle(nx, ny, tau=1.1, tau_g=tau_g, T_bottom=Tb, T_top=Tt, T_ref=Tref, alpha_g=0.0)
+        Tl = (Tb + (Tt - Tb) * (np.arange(ny) + 0.5) / ny)[:, None].repeat(nx, 1)
+        f = _linear_pops(np.full((ny, nx), 0.5), 0.0, U)
+        o2.set_populations(f, 1.4 * f, _linear_pops(Tl, 0.0, 0.0))
+        assert o2.observables()["Nu"] == pytest.approx(1 + U * 0.5 * (Tb + Tt) * ny / (kappa * dT), rel=1e-12)
+
+
+def test_x_average_with_posts_closed_form(oracle_mod):
+    """u_av[y] (L248-250) = mean over the FLUID sites of row y of u_x^(H); rows through the posts average over
+    the gaps only, rows without fluid report 0."""
+    nx, ny = 32, 12
+    solid = inputs.post_mask(nx, ny, 5, 3, 8)
+    solid[ny // 2, :] = 1  # one row without any fluid site
+    o = oracle_mod.Oracle(nx, ny, tau=1.0, thermal=0)
+    o.set_solid(solid)
+    rA, rB, T, UA, UB = _flow_state(nx, ny, 33)
+    fl = solid == 0
+    o.set_populations(_linear_pops(rA, *UA) * fl, _linear_pops(rB, *UB) * fl, 0 * _linear_pops(T, 0, 0))
+    ux = (rA * UA[0] + rB * UB[0]) / (rA + rB)
+    expect = np.array([ux[y][fl[y]].mean() if fl[y].any() else 0.0 for y in range(ny)])
+    got = o.x_average()
+    assert np.abs(got - expect).max() < 1e-15
+    assert got[ny // 2] == 0.0
+    assert np.abs(ux.mean(1) - expect)[:3].max() > 1e-4  # averaging over all nx sites would differ on post rows
