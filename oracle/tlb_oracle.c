@@ -10,7 +10,7 @@
  *
  * The method is an explicit iteration, so the oracle follows it step by step in the
  * paper's order and notation (PAPER Eqs. (1)-(22)); readings of silent / garbled passages
- * are the ones listed in DESIGN.md ("Readings R1..R19").  No blocking, fusion or reordering:
+ * are the ones listed in DESIGN.md ("Readings R1..R22").  No blocking, fusion or reordering:
  * every sub-step is a full sweep over the lattice writing a full array.
  *
  * Parity pins (tests/test_oracle_pins.py, all run with -m "not gpu"):
@@ -26,6 +26,12 @@
  *   observables        mass, E and the convective term of Nu against closed forms on states with
  *                      known moments (random masks, posts, buoyancy so that u^(H) != u);
  *                      u_av on rows through posts                            L248, Eq. (24)
+ *   stress P_xy        exact -rho nu (U_t - U_b)/ny in single-phase Couette for three tau; Pxy_av constant across
+ *                      the interface of a sheared two-layer state; exact row-by-row momentum balance of one step
+ *                      on a random two-component state (interaction part, NN couplings) and its first moment
+ *                      (all couplings)                                       L248-250, L294-296, Eq. (14) (R21)
+ *   droplets           hand-made masks with known clusters, a droplet across the x seam, exact centroids of
+ *                      discs, invariance under x shifts                      section 2.4 L198 (R22)
  *   posts / corners    second, independently written streaming formulation
  *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
  *                      pull of orc_step; beyond that and mass conservation the post-corner
@@ -450,6 +456,130 @@ void orc_x_average(orc_state *s, double *u_av) {
       if (!s->solid[IDX(s, x, y)]) { a += s->uHx[IDX(s, x, y)]; n++; }
     u_av[y] = n ? (double)(a / n) : 0.0;
   }
+}
+
+/* Stress field P_xy (the paper's Ptot_xy.dat, L248-250; "the sum of all components contributions", L296).
+ * The paper prints no formula; reading R21:
+ *   kinetic part      sum_l (1/2) sum_i c_ix c_iy (f_l,i + f*_l,i): the momentum flux carried by the populations
+ *                     that arrive at the site (f, time t) and by those that leave it (f*, post-collision, Eq. (2))
+ *   interaction part  for every pairwise force F(x) = -G psi(x) sum_c k(c) psi'(x+c) c of Eqs. (7), (10), (11)
+ *                     the tensor (G/2) psi(x) sum_c k(c) psi'(x+c) c_x c_y, wall values at solid nodes (L155)
+ * 0 on solid sites.  Sign: pressure tensor, P_xy = -eta d_y u_x in a simple shear (L143). */
+void orc_stress_xy(orc_state *s, double *Pxy) {
+  const int nx = s->nx, ny = s->ny;
+  const orc_params *p = &s->p;
+  moments_and_forces(s);
+  collide(s);
+  const double psx_wA = psi_x_of(s, p->rho_wall_A), psx_wB = psi_x_of(s, p->rho_wall_B);
+  const double pss_wA = psi_s_of(s, p->rho_wall_A), pss_wB = psi_s_of(s, p->rho_wall_B);
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      size_t k = IDX(s, x, y);
+      if (s->solid[k]) { Pxy[k] = 0.0; continue; }
+      double kin = 0.0;
+      for (int i = 0; i < 9; i++) {
+        size_t q = PIDX(s, i, x, y);
+        kin += 0.5 * (CX[i] * CY[i]) * ((s->fA[q] + s->fAs[q]) + (s->fB[q] + s->fBs[q]));
+      }
+      double cross = 0.0, selfA = 0.0, selfB = 0.0;
+      for (int dy = -2; dy <= 2; dy++)
+        for (int dx = -2; dx <= 2; dx++) {
+          int c2 = dx * dx + dy * dy;
+          if (c2 == 0) continue;
+          int xx = x + dx, yy = y + dy;
+          double nxA, nxB, nsA, nsB;
+          if (is_solid(s, xx, yy)) { nxA = psx_wA; nxB = psx_wB; nsA = pss_wA; nsB = pss_wB; }
+          else {
+            size_t kk = IDX(s, wrap(xx, nx), p->periodic_y ? wrap(yy, ny) : yy);
+            nxA = s->psxA[kk]; nxB = s->psxB[kk]; nsA = s->pssA[kk]; nsB = s->pssB[kk];
+          }
+          double w = w_of_c2(c2), pp = p_of_c2(c2);
+          cross += w * (s->psxA[k] * nxB + s->psxB[k] * nxA) * (dx * dy);
+          selfA += (p->G11a * w + p->G11r * pp) * s->pssA[k] * nsA * (dx * dy);
+          selfB += (p->G22a * w + p->G22r * pp) * s->pssB[k] * nsB * (dx * dy);
+        }
+      Pxy[k] = kin + 0.5 * (p->G12 * cross + selfA + selfB);
+    }
+}
+
+/* x-average over the fluid sites of every row of a field plane (Pxy_av.dat, L250); 0 for a row without fluid. */
+void orc_row_average(const orc_state *s, const double *plane, double *av) {
+  for (int y = 0; y < s->ny; y++) {
+    long double a = 0;
+    long n = 0;
+    for (int x = 0; x < s->nx; x++)
+      if (!s->solid[IDX(s, x, y)]) { a += plane[IDX(s, x, y)]; n++; }
+    av[y] = n ? (double)(a / n) : 0.0;
+  }
+}
+
+/* x-momentum of every row, sum over x, both species and all directions of c_ix f_l,i (the conserved quantity
+ * the stress pins balance). */
+void orc_row_momentum_x(const orc_state *s, double *mx) {
+  for (int y = 0; y < s->ny; y++) {
+    long double a = 0;
+    for (int x = 0; x < s->nx; x++)
+      for (int i = 0; i < 9; i++) a += CX[i] * (s->fA[PIDX(s, i, x, y)] + s->fB[PIDX(s, i, x, y)]);
+    mx[y] = (double)a;
+  }
+}
+
+/* Droplet analysis, first stage (section 2.4; reading R22): bulk sites are the fluid sites with
+ * rho_A > B_th; a droplet is a cluster of bulk sites connected through nearest-neighbour bonds (the bonds of the
+ * Ising cluster algorithms the paper adapts, L198), x periodic, y periodic iff periodic_y.  Plain flood fill in
+ * site-index order, so a cluster's label is its smallest site index y nx + x; -1 off the bulk.
+ * stats[k] = {label, sites, centre x, centre y} in ascending label order, the centre being the mean position of
+ * the cluster's sites: integer sums of minimum-image offsets from the label site (signed, in [-n/2, n/2)),
+ * one division, wrapped to [0, nx) (and [0, ny) when y is periodic).  Returns the number of droplets; only the
+ * first max_droplets rows of stats are written. */
+static int min_image(int a, int b, int n) {
+  int d = a - b;
+  if (2 * d >= n) d -= n;
+  else if (2 * d < -n) d += n;
+  return d;
+}
+int orc_droplets(orc_state *s, double B_th, int32_t *labels, int max_droplets, double *stats) {
+  const int nx = s->nx, ny = s->ny;
+  const size_t n = (size_t)nx * ny;
+  moments_and_forces(s);
+  int32_t *lab = labels ? labels : (int32_t *)malloc(n * sizeof(int32_t));
+  int *stack = (int *)malloc(n * sizeof(int));
+  for (size_t k = 0; k < n; k++) lab[k] = (!s->solid[k] && s->rhoA[k] > B_th) ? -2 : -1; /* -2: bulk, unvisited */
+  int found = 0;
+  for (size_t k = 0; k < n; k++) {
+    if (lab[k] != -2) continue;
+    const int xr = (int)(k % nx), yr = (int)(k / nx);
+    long long cnt = 0, sdx = 0, sdy = 0;
+    int top = 0;
+    stack[top++] = (int)k;
+    lab[k] = (int32_t)k;
+    while (top) {
+      const int q = stack[--top], x = q % nx, y = q / nx;
+      cnt++;
+      sdx += min_image(x, xr, nx);
+      sdy += s->p.periodic_y ? min_image(y, yr, ny) : y - yr;
+      const int nbx[4] = {wrap(x + 1, nx), wrap(x - 1, nx), x, x};
+      int nby[4] = {y, y, y + 1, y - 1};
+      for (int b = 0; b < 4; b++) {
+        if (s->p.periodic_y) nby[b] = wrap(nby[b], ny);
+        else if (nby[b] < 0 || nby[b] >= ny) continue;
+        const size_t m = IDX(s, nbx[b], nby[b]);
+        if (lab[m] == -2) { lab[m] = (int32_t)k; stack[top++] = (int)m; }
+      }
+    }
+    if (found < max_droplets) {
+      double cx = (double)xr + (double)sdx / (double)cnt, cy = (double)yr + (double)sdy / (double)cnt;
+      if (cx < 0.0) cx += nx;
+      if (cx >= nx) cx -= nx;
+      if (s->p.periodic_y) { if (cy < 0.0) cy += ny; if (cy >= ny) cy -= ny; }
+      stats[4 * found + 0] = (double)k; stats[4 * found + 1] = (double)cnt;
+      stats[4 * found + 2] = cx; stats[4 * found + 3] = cy;
+    }
+    found++;
+  }
+  free(stack);
+  if (!labels) free(lab);
+  return found;
 }
 
 /* lattice constants exported for the weight-invariant pins */

@@ -54,6 +54,11 @@ def _load():
         lib.orc_forces.argtypes = [ctypes.c_void_p, dp, dp]
         lib.orc_observables.argtypes = [ctypes.c_void_p, dp]
         lib.orc_x_average.argtypes = [ctypes.c_void_p, dp]
+        lib.orc_stress_xy.argtypes = [ctypes.c_void_p, dp]
+        lib.orc_row_average.argtypes = [ctypes.c_void_p, dp, dp]
+        lib.orc_row_momentum_x.argtypes = [ctypes.c_void_p, dp]
+        lib.orc_droplets.restype = ctypes.c_int
+        lib.orc_droplets.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p, ctypes.c_int, dp]
         lib.orc_w.restype = ctypes.c_double
         lib.orc_w.argtypes = [ctypes.c_int, ctypes.c_int]
         lib.orc_p.restype = ctypes.c_double
@@ -148,6 +153,41 @@ def _x_average(self):
 
 
 Oracle.x_average = _x_average
+
+
+def _stress_xy(self):
+    """P_xy [ny][nx] (reading R21)."""
+    out = np.empty((self.ny, self.nx))
+    self.lib.orc_stress_xy(self.h, _dp(out))
+    return out
+
+
+def _x_average_stress(self):
+    """Pxy_av[ny]: x-average of P_xy over the fluid sites of each row."""
+    pxy = _stress_xy(self)
+    out = np.empty(self.ny)
+    self.lib.orc_row_average(self.h, _dp(pxy), _dp(out))
+    return out
+
+
+def _row_momentum_x(self):
+    out = np.empty(self.ny)
+    self.lib.orc_row_momentum_x(self.h, _dp(out))
+    return out
+
+
+def _droplets(self, B_th, max_droplets):
+    """(labels [ny][nx] int32, n_droplets, stats [min(n, max)][4]) -- section 2.4, reading R22."""
+    labels = np.empty((self.ny, self.nx), dtype=np.int32)
+    stats = np.zeros((max(1, max_droplets), 4))
+    n = self.lib.orc_droplets(self.h, float(B_th), labels.ctypes.data, int(max_droplets), _dp(stats))
+    return labels, n, stats[:min(n, max_droplets)]
+
+
+Oracle.stress_xy = _stress_xy
+Oracle.x_average_stress = _x_average_stress
+Oracle.row_momentum_x = _row_momentum_x
+Oracle.droplets = _droplets
 
 
 def lattice_weights():
