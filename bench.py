@@ -7,10 +7,13 @@ A "step" is one lattice-Boltzmann time step (rows a1-a9 of SURVEY.md section 8: 
 force+collide+stream kernel + boundary kernel) over the whole lattice of the workload.  Default
 workload: BASELINE.json configs[3], the 4096x2048 headline config (4000 droplets r = 14, 4x4 posts
 period 16 on both walls, thermal + buoyancy, fp64), synthetic seeded input.
-N > 1 (torchrun): every rank advances its own replica of the workload (different seed), no
-data-path collective ("replicas only", DESIGN.md section Multi-GPU); value = all ranks' site updates
-over the max-over-ranks device time.
+N > 1 (torchrun): the lattice is split into N contiguous y-slabs, one process per GPU; per step and interior
+face the 3 rows next to the face travel to the neighbour (NCCL point-to-point on a side stream, overlapped with
+the interior rows; DESIGN.md section 8).  Default: the SAME lattice split N ways ("scaling": "strong");
+--scaling weak stacks N copies of the workload in y (ny = N * ny of the config).  value = all site updates over the
+max-over-ranks device time.
 """
+import hashlib
 import argparse
 import json
 import os
@@ -36,11 +39,24 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
 
 
+def kernel_source_hash():
+    """sha256 of the sources that define the fused kernel (what a committed ncu capture is valid for)."""
+    h = hashlib.sha256()
+    for f in ("tlb_step.cu", "tlb_internal.cuh"):
+        with open(os.path.join(ROOT, "paper_2109_12565_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()
+
+
 def committed_traffic(name):
-    """dram bytes per fused-kernel launch from the committed ncu --set full summary, or None."""
+    """dram bytes per fused-kernel launch from the committed ncu --set full summary (profiles/traffic.json), or None
+    when there is no capture for this workload or the kernel sources have changed since it was taken."""
     try:
         with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            return json.load(f).get(name)
+            e = json.load(f).get(name)
+        if not isinstance(e, dict) or e.get("kernel_source_sha256") != kernel_source_hash():
+            return None
+        return e["dram_bytes_per_launch"]
     except Exception:
         return None
 
@@ -145,15 +161,15 @@ def run_ours(args, rank, world):
     local = int(os.environ.get("LOCAL_RANK", 0))
     torch.cuda.set_device(local)
     dev = "cuda:%d" % local
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
     binding.load_library()  # raises if libtlb.so is missing
+    if world > 1:
+        return run_slabs(args, rank, world, local)
     cfg = inputs.config(args.config)
     nx, ny = cfg["nx"], cfg["ny"]
     sites = nx * ny
     alg_bytes = ALG_BYTES_PER_SITE * args.pop_precision // 64  # 432 B (fp64 storage) or 216 B (fp32 storage)
     t = binding.TLB(nx, ny, params=binding.params_from_config(cfg), device=dev, pop_precision=args.pop_precision)
-    t.init(replicas.rank_seed(cfg["seed"], rank))
+    t.init(cfg["seed"])
 
     def barrier():
         if world > 1:
@@ -195,6 +211,26 @@ def run_ours(args, rank, world):
                 "kernel_share_of_step": fused_ms / step_ms}
     ob = t.observables()
     finite = all(v == v and abs(v) != float("inf") for v in ob.values())
+    u = t.fields()[2]
+    umax = float((u[0] * u[0] + u[1] * u[1]).max().sqrt())  # print max |u^(H)| of every run
+    del u
+
+    # ---- optional long run with the observables logged (BASELINE config 2: Nu and mass every 1000 steps)
+    obs_log = None
+    if args.observe_every > 0:
+        t.init(cfg["seed"])
+        m0 = t.observables()
+        obs_log = []
+        for k in range(args.observe_every, cfg["steps"] + 1, args.observe_every):
+            t.step(args.observe_every)
+            o = t.observables()
+            uu = t.fields()[2]
+            obs_log.append({"step": k, "Nu": o["Nu"], "mass_A": o["mass_A"], "mass_B": o["mass_B"], "E": o["E"],
+                            "mass_A_drift": o["mass_A"] / m0["mass_A"] - 1, "mass_B_drift": o["mass_B"] / m0["mass_B"] - 1,
+                            "max_uH": float((uu[0] * uu[0] + uu[1] * uu[1]).max().sqrt())})
+            print("step %6d  Nu %.9f  mass_A %.12e (%+.2e)  mass_B %.12e (%+.2e)  max|uH| %.4e"
+                  % (k, o["Nu"], o["mass_A"], obs_log[-1]["mass_A_drift"], o["mass_B"], obs_log[-1]["mass_B_drift"],
+                     obs_log[-1]["max_uH"]), file=sys.stderr)
 
     # ---- end to end through the host-buffer ABI: per step H2D of the three input fields from pinned
     # memory, one LB step, D2H of the four observables
@@ -217,6 +253,23 @@ def run_ours(args, rank, world):
            "d2h_bytes_per_step": 32, "steps": e2e_steps,
            "call": "tlb_set_fields_host + tlb_step(1) + tlb_observables_host per step"}
     del solid_h
+    # the same with the step's full result read back: tlb_fields_host(rho_A, rho_B, u, T), 5 planes
+    ha, hb, ht = (torch.empty((ny, nx), dtype=torch.float64).pin_memory() for _ in range(3))
+    hu = torch.empty((2, ny, nx), dtype=torch.float64).pin_memory()
+    for _ in range(2):
+        t.set_fields_host(fa, fb, ft); t.step(1); t.fields_host(ha, hb, hu, ht)
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        t.set_fields_host(fa, fb, ft)
+        t.step(1)
+        t.fields_host(ha, hb, hu, ht)
+    torch.cuda.synchronize()
+    e2f_ms = (time.perf_counter() - w0) * 1e3
+    e2e_fields = {"value": sites * e2e_steps / e2f_ms / 1e3, "unit": "MLUPS", "h2d_bytes_per_step": 3 * 8 * sites,
+                  "d2h_bytes_per_step": 5 * 8 * sites, "steps": e2e_steps,
+                  "call": "tlb_set_fields_host + tlb_step(1) + tlb_fields_host(rho_A, rho_B, u, T) per step"}
+    del ha, hb, ht, hu
 
     # ---- CPU baseline: the oracle as it stands on this host, rank 0 at N = 1 only
     cpu = None
@@ -237,11 +290,101 @@ def run_ours(args, rank, world):
                        "posts": list(cfg["posts"]), "state_bytes": alg_bytes // 2 * sites, "pop_precision": args.pop_precision,
                        "l2": "state (%.2f GB per buffer) exceeds the 126 MB L2; no flush needed" % (216 * sites / 1e9)
                        if 216 * sites > 4 * 126e6 else "state fits in L2: HBM figures are not meaningful",
-                       "parallelism": "replicas x%d" % world, "finite": finite, "mass_A": ob["mass_A"], "Nu": ob["Nu"]},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+                       "parallelism": "1 GPU, whole lattice", "finite": finite, "mass_A": ob["mass_A"], "Nu": ob["Nu"],
+                       "max_uH": umax},
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_fields": e2e_fields, "observables_log": obs_log,
+            "gpu_launches": launches, "clocks": clocks,
             "effective_GBs": alg_bytes * mlups / 1e3, "roofline_frac_whole_step": alg_bytes * mlups / 1e3 / peak / world}))
-    if world > 1:
-        dist.destroy_process_group()
+
+
+def run_slabs(args, rank, world, local):
+    """N > 1: y-slab decomposition, one process per GPU."""
+    import torch
+    import torch.distributed as dist
+    from paper_2109_12565_b200 import binding, inputs, replicas, slabs
+
+    dev = "cuda:%d" % local
+    dist.init_process_group("nccl", device_id=torch.device(dev))
+    cfg = inputs.config(args.config)
+    nx = cfg["nx"]
+    ny = cfg["ny"] * (world if args.scaling == "weak" else 1)
+    par = binding.params_from_config(cfg)
+    if args.scaling == "weak":
+        par.n_droplets = cfg["init"]["n_droplets"] * world  # the same emulsion, N times as tall
+    alg_bytes = ALG_BYTES_PER_SITE * args.pop_precision // 64
+    s = slabs.DistributedSlab(nx, ny, params=par, device=dev, pop_precision=args.pop_precision)
+    s.init(cfg["seed"])
+    own_sites = nx * (s.y1 - s.y0)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    s.step(max(3, args.warmup))
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    l0 = s.t.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(s.t.stream)
+    s.step(args.steps)
+    e1.record(s.t.stream)
+    barrier()
+    launches = s.t.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.summary()
+    mlups, ms = replicas.aggregate_mlups(own_sites, args.steps, ms, dev)  # all slabs' updates / max-over-ranks time
+    launches = int(replicas.sum_over_ranks(launches, dev))
+    ob = s.observables()
+    finite = all(v == v and abs(v) != float("inf") for v in ob.values())
+    peak, peak_src = measured_peak()
+    step_ms = ms / args.steps
+    achieved = alg_bytes * own_sites / step_ms / 1e6  # this rank's bytes over the slowest rank's step: a lower bound
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false, %s>" % ("double" if args.pop_precision == 64 else "float"),
+                "kernel_ms": step_ms, "method": "per GPU: own rows x alg. bytes / whole step time (edges + interior + halo "
+                "exchange + boundary kernel), max over ranks", "alg_bytes_per_launch": alg_bytes * own_sites}
+
+    # ---- end to end: per step H2D of this slab's three input fields, one step with its halo exchange, the observables
+    # all-reduced and read back
+    nyl = s.t.ny
+    fa, fb, ft = (torch.empty((nyl, nx), dtype=torch.float64).pin_memory() for _ in range(3))
+    s.t.fields_host(fa, fb, None, ft)
+    e2e_steps = max(3, min(args.steps, 20))
+    # tlb_fields_host writes the owned rows only; a slab's state-setting calls take the halo rows from the caller's
+    # arrays: repeat the nearest owned row there
+    for h in (fa, fb, ft):
+        h[:s.t.own0] = h[s.t.own0]
+        h[s.t.own1:] = h[s.t.own1 - 1]
+    for _ in range(2):
+        s.t.set_fields_host(fa, fb, ft); s.step(1); s.observables()
+    barrier()
+    w0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        s.t.set_fields_host(fa, fb, ft)
+        s.step(1)
+        s.observables()
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - w0) * 1e3
+    e2e_mlups, _ = replicas.aggregate_mlups(own_sites, e2e_steps, e2e_ms, dev)
+    e2e = {"value": e2e_mlups, "unit": "MLUPS", "h2d_bytes_per_step": int(replicas.sum_over_ranks(3 * 8 * nx * nyl, dev)),
+           "d2h_bytes_per_step": 32 * world, "steps": e2e_steps,
+           "call": "per rank: tlb_set_fields_host + slab step (edges, pack, interior, NCCL exchange, unpack, finish) + "
+                   "tlb_observable_sums, all-reduce, tlb_observables_from_sums"}
+    if rank == 0:
+        print(json.dumps({
+            "metric": "MLUPS", "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": max(3, args.warmup), "ms_per_step": step_ms, "higher_is_better": True, "scaling": args.scaling,
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg["name"] + ("" if args.scaling == "strong" else "_x%d_in_y" % world), "nx": nx, "ny": ny,
+                       "posts": list(cfg["posts"]), "pop_precision": args.pop_precision,
+                       "parallelism": "%d y-slabs, halo exchange of 3 rows x 27 planes per face and step (NCCL p2p)" % world,
+                       "l2": "state exceeds L2; no flush needed" if 216 * own_sites > 4 * 126e6 else
+                             "a slab's state fits in L2: HBM figures are not meaningful",
+                       "finite": finite, "mass_A": ob["mass_A"], "Nu": ob["Nu"]},
+            "roofline": roofline, "cpu_baseline": None, "e2e": e2e, "gpu_launches": launches, "clocks": clocks,
+            "effective_GBs": alg_bytes * mlups / 1e3, "roofline_frac_whole_step": alg_bytes * mlups / 1e3 / peak / world}))
+    dist.destroy_process_group()
 
 
 def main():
@@ -252,6 +395,10 @@ def main():
     ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
+                    help="N > 1: split the config's lattice into N y-slabs (strong) or stack N copies of it in y (weak)")
+    ap.add_argument("--observe-every", type=int, default=0,
+                    help="also run the config's full step count from its initial state, logging Nu / mass / max|uH| every so many steps")
     ap.add_argument("--pop-precision", type=int, default=64, choices=[64, 32],
                     help="storage of the populations in HBM (32: bandwidth study of BASELINE config 5; arithmetic stays fp64)")
     args = ap.parse_args()

@@ -3,7 +3,7 @@
  *
  * The operation is the per-time-step update of TLBfind (arXiv 2109.12565); citations are
  * "PAPER L<line>" into /root/reference/PAPER.md plus the equation / section they fall in.
- * Readings R1..R19 of silent or garbled passages are listed in DESIGN.md.
+ * Readings R1..R22 of silent or garbled passages are listed in DESIGN.md.
  *
  * One step (tlb_step) computes, for every fluid site, from time-t populations only (R13):
  *   moments            rho_l = sum_i f_l,i ; T = sum_i g_i ; j = sum_l,i c_i f_l,i     Eqs. (4),(5),(17) L76-80, L165
@@ -33,8 +33,31 @@
  *   `workspace` and `stream` given to tlb_create, which must outlive the handle.
  *   Asynchrony: device-pointer calls enqueue on the handle's stream and return; *_host calls and
  *   tlb_observables_host return after the stream has been synchronised.
- *   Errors: every call returns 0 (TLB_OK) or a negative code, never aborts or throws.
+ *   Errors: every call returns 0 (TLB_OK) or a negative code, never aborts or throws.  A CUDA error raised by
+ *   the handle's own work is sticky on the handle (TLB_ECUDA from then on).  A CUDA error that some other
+ *   library left pending on the calling thread makes a call return TLB_ECUDA without doing anything and
+ *   without consuming or adopting that error.
+ *   Device: the handle lives on the CUDA device that owns `workspace`; every entry point makes that device
+ *   current for its duration and restores the caller's, so a multi-GPU host process may switch devices freely.
+ *   `stream` must be a stream of that device.
  *   There is no CPU fallback: without a CUDA device tlb_create returns TLB_ECUDA.
+ *
+ * Y-SLABS (multi-GPU, the paper's stated future work L376)
+ *   tlb_create_slab makes a handle for rows [y0, y1) of an nx x ny lattice.  Its local lattice has
+ *   ny_local = (y1 - y0) + halo_lo + halo_hi rows: 3 halo rows beyond every face that is not a flat wall of
+ *   the whole lattice (with periodic_y every face has them and row indices wrap).  Every array argument of a
+ *   slab handle is [ny_local][nx] (or [9][ny_local][nx]), local row r being row (y0 - halo_lo + r) of the
+ *   whole lattice; state-setting calls take the halo rows from the caller's arrays, output calls write the
+ *   owned rows only.  One time step is
+ *       tlb_slab_step_edges     fused kernel on the 3 owned rows next to each halo face
+ *       tlb_halo_pack(face)     those rows of all 27 planes -> a contiguous buffer of tlb_halo_bytes
+ *       tlb_slab_step_interior  fused kernel on the remaining owned rows (overlaps the exchange)
+ *       ... the caller moves each packed buffer to the neighbour across that face (NCCL, peer copy) ...
+ *       tlb_halo_unpack(face)   neighbour's buffer -> the halo rows beyond `face`
+ *       tlb_slab_step_finish    boundary kernel over every solid node of the local lattice; state advances
+ *   (3 rows: the pull of the 2 force-stencil rows beyond a face reaches one row further.)  The result is bit
+ *   for bit that of one handle on the whole lattice.  tlb_observable_sums gives a slab's share of the six
+ *   sums behind tlb_observables; after an all-reduce tlb_observables_from_sums finishes them.
  */
 #ifndef TLB_H
 #define TLB_H
@@ -68,7 +91,9 @@ typedef struct tlb_params {
   double droplet_radius, min_gap, rho_in, rho_out, noise_amp;
   int32_t n_droplets;
   int32_t periodic_y;                 /* 0: walls (default); 1: periodic in y (L147, L284-302)              */
-  int32_t thermal;                    /* THERMAL switch, L314: 0 leaves g untouched and uses T = T_ref      */
+  int32_t thermal;                    /* THERMAL switch, L314: 0 leaves g untouched (the step neither reads */
+                                      /* nor writes it) and the buoyancy uses T = T_ref; tlb_fields and Nu  */
+                                      /* still report sum_i g_i of the frozen populations                   */
   int32_t post_w, post_h, post_period;/* structured rough walls used by tlb_init (R19); 0,0,0 = smooth      */
   int32_t pop_precision;              /* storage of the populations in HBM: 64 (default) or 32 (bandwidth   */
                                       /* study of BASELINE config 5; the arithmetic stays fp64)             */
@@ -94,6 +119,19 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
                void* stream, tlb_handle** out);
 int tlb_destroy(tlb_handle* h);
 
+/* Y-slab handle for rows [y0, y1) of the nx x ny lattice (see Y-SLABS above).  TLB_EINVAL additionally for
+ * y0 < 0, y1 > ny, y1 <= y0, or fewer than 3 owned rows next to a halo face. */
+int tlb_slab_workspace_bytes(int nx, int ny, int y0, int y1, const tlb_params* p, size_t* bytes);
+int tlb_create_slab(int nx, int ny, int y0, int y1, const tlb_params* p, void* workspace, size_t workspace_bytes,
+                    void* stream, tlb_handle** out);
+/* out6 = { ny_local, own0, own1, y_off, halo_lo, halo_hi }: owned local rows [own0, own1); local row r is row
+ * y_off + r of the whole lattice (wrapped when periodic_y).  A whole-lattice handle reports {ny, 0, ny, 0, 0, 0}. */
+int tlb_slab_layout(const tlb_handle* h, int32_t out6[6]);
+/* Bytes of one packed halo face: 27 planes x 3 padded rows in the storage precision. */
+int tlb_halo_bytes(const tlb_handle* h, size_t* bytes);
+/* Rows per CTA segment of the fused kernel's launch (so that tests can aim at a segment edge). */
+int tlb_seg_rows(const tlb_handle* h);
+
 /* Seeded initial state of the input recipe: structured posts from params, n_droplets
  * discs by random sequential addition, +noise, linear T profile (L314), populations at rest
  * equilibrium f = w rho, g = w T (R14).  Bit-identical to paper_2109_12565_b200/inputs.py. */
@@ -114,10 +152,21 @@ int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, 
 int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g);
 
 /* Advance n >= 0 time steps (n = 0 is a no-op): per step one fused force+collide+stream kernel and
- * one wall/obstacle boundary kernel.  Whole blocks of 16 steps are replayed from a CUDA graph captured on
- * first use (one launch instead of 32; matters for launch-bound lattices); the rest is launched kernel by
- * kernel.  Set the environment variable TLB_NO_GRAPH to disable the graphs. */
+ * one wall/obstacle boundary kernel.  Whole blocks of 16 steps are replayed from a CUDA graph (one launch
+ * instead of 32; matters for launch-bound lattices); the rest is launched kernel by kernel.  The graphs are
+ * captured by the first call with n > 0 after the obstacle mask was set, before it enqueues anything.
+ * TLB_EINVAL on a slab handle that has halo rows. */
 int tlb_step(tlb_handle* h, int64_t n);
+
+/* One time step of a y-slab in four parts (see Y-SLABS above); device pointers, all on the handle's stream.
+ * face 0 = low y, 1 = high y; TLB_EINVAL for a face without halo rows.  While a step is open (after _edges,
+ * before _finish) pack / unpack address the buffer being written, otherwise the current state.
+ * TLB_ESTATE when called out of order. */
+int tlb_slab_step_edges(tlb_handle* h);
+int tlb_slab_step_interior(tlb_handle* h);
+int tlb_slab_step_finish(tlb_handle* h);
+int tlb_halo_pack(tlb_handle* h, int face, void* buf);
+int tlb_halo_unpack(tlb_handle* h, int face, const void* buf);
 
 /* Measurement aid: advance ONE step, launching the fused kernel n (1..4096) times back to back on the
  * same input / output buffers and then the boundary kernel n times (both are idempotent on fixed inputs),
@@ -134,15 +183,47 @@ int tlb_fields_host(tlb_handle* h, double* rho_A, double* rho_B, double* u, doub
 /* out[4] = { mass_A, mass_B, E, Nu }: mass_l = sum over fluid sites of rho_l (north_star);
  * E = mean over fluid sites of |u^(H)|^2 (L248, R11); Nu of Eq. (24) L347 in the reading R10.
  * tlb_observables writes to a DEVICE pointer; tlb_observables_host to a HOST pointer (synchronises).
- * Deterministic: warp-shuffle block partials combined in a fixed order. */
+ * One pass over the populations: the fused kernel reduces inside each CTA with warp shuffles, a second
+ * small kernel combines the CTAs; fixed order, deterministic.  TLB_EINVAL on a slab handle with halo rows:
+ * tlb_observable_sums writes the slab's share sums6 = { mass_A, mass_B, sum |u^(H)|^2, sum u_y^(H) T,
+ * sum d_y T, fluid sites } (DEVICE), and tlb_observables_from_sums turns the all-reduced sums into out4. */
 int tlb_observables(tlb_handle* h, double* out4);
 int tlb_observables_host(tlb_handle* h, double* out4);
+int tlb_observable_sums(tlb_handle* h, double* sums6);
+int tlb_observables_from_sums(tlb_handle* h, const double* sums6, double* out4);
 
 /* u_av[ny] (DEVICE pointer; _host: HOST pointer, synchronises): the x-average over the fluid sites of every
  * row of u_x^(H), the profile the paper dumps as u_av.dat for the Couette rheology (L248-250, Eq. (23));
  * 0 for a row without fluid sites.  Deterministic (one CTA per row, fixed-order sums). */
 int tlb_x_average(tlb_handle* h, double* u_av);
 int tlb_x_average_host(tlb_handle* h, double* u_av);
+
+/* P_xy [ny][nx]: the off-diagonal component of the total stress (pressure-tensor sign: P_xy = -eta du_x/dy in a
+ * simple shear) that the paper dumps as Ptot_xy.dat and, x-averaged over the fluid sites of each row, as
+ * Pxy_av.dat [ny] for the rheology (L248-250, Eq. (23)).  The paper gives no formula; reading
+ * R21: "the sum of all components contributions" (L296) =
+ *   sum_l 1/2 sum_i c_ix c_iy (f_l,i + f*_l,i)                the momentum flux carried by the populations that
+ *                                                             arrive at and leave the site (f*: post-collision)
+ * + 1/2 sum_c c_x c_y [ G12 (psi^x_A(x) w(c) psi^x_B(x+c) + psi^x_B(x) w(c) psi^x_A(x+c))
+ *                       + sum_l psi^s_l(x) (G_ll^a w(c) + G_ll^r p(c)) psi^s_l(x+c) ]   the interaction part of
+ *                                                             Eqs. (7), (10), (11) (wall values at solid nodes).
+ * 0 at solid sites.  Same conventions as tlb_fields / tlb_x_average. */
+int tlb_stress_xy(tlb_handle* h, double* P_xy);
+int tlb_stress_xy_host(tlb_handle* h, double* P_xy);
+int tlb_x_average_stress(tlb_handle* h, double* Pxy_av);
+int tlb_x_average_stress_host(tlb_handle* h, double* Pxy_av);
+
+/* Droplet analysis, first stage (section 2.4; reading R22): bulk sites = fluid sites with rho_A > B_th;
+ * droplets = clusters of nearest-neighbour (4-connected) bulk sites, x periodic (y too with periodic_y).
+ *   labels     [ny][nx] int32 or NULL: smallest site index (y nx + x) of the site's cluster, -1 off the bulk
+ *   n_droplets the number of droplets found
+ *   stats      [max_droplets][4] = { label, sites, centre x, centre y } in ascending label order; the centre is
+ *              the mean position of the cluster's sites (minimum image in x from the label site, wrapped to
+ *              [0, nx)).  Meaningful only if n_droplets <= max_droplets.
+ * Integer / index work: every output is bit-identical to the oracle's flood fill.  DEVICE pointers; _host: HOST
+ * pointers (synchronises).  TLB_EINVAL on slab handles and for max_droplets > nx ny / 4. */
+int tlb_droplets(tlb_handle* h, double B_th, int32_t* labels, int32_t max_droplets, int32_t* n_droplets, double* stats);
+int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_droplets, int32_t* n_droplets, double* stats);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t tlb_launch_count(const tlb_handle* h);

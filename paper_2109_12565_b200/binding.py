@@ -11,7 +11,7 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
-LIB_PATH = os.environ.get("TLB_LIB") or os.path.join(_HERE, "libtlb.so")  # TLB_LIB: A/B experiments only
+LIB_PATH = os.path.join(_HERE, "libtlb.so")
 SOURCES = ["tlb_step.cu", "tlb_aux.cu", "tlb_api.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
@@ -19,13 +19,15 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
 TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT = 0, -1, -2, -3, -4
 
 # every symbol include/tlb.h declares
-SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_init", "tlb_set_solid",
+SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_slab_workspace_bytes",
+           "tlb_create_slab", "tlb_slab_layout", "tlb_halo_bytes", "tlb_seg_rows", "tlb_init", "tlb_set_solid",
            "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
            "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step",
-           "tlb_profile_step", "tlb_fields",
-           "tlb_fields_host", "tlb_observables", "tlb_observables_host", "tlb_x_average", "tlb_x_average_host",
-           "tlb_launch_count", "tlb_error_string",
-           "tlb_last_cuda_error"]
+           "tlb_slab_step_edges", "tlb_slab_step_interior", "tlb_slab_step_finish", "tlb_halo_pack", "tlb_halo_unpack",
+           "tlb_profile_step", "tlb_fields", "tlb_fields_host", "tlb_observables", "tlb_observables_host",
+           "tlb_observable_sums", "tlb_observables_from_sums", "tlb_x_average", "tlb_x_average_host",
+           "tlb_stress_xy", "tlb_stress_xy_host", "tlb_x_average_stress", "tlb_x_average_stress_host",
+           "tlb_droplets", "tlb_droplets_host", "tlb_launch_count", "tlb_error_string", "tlb_last_cuda_error"]
 
 
 class TLBParams(ctypes.Structure):
@@ -58,8 +60,7 @@ def build(force=False, verbose=False):
         return LIB_PATH
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     tmp = LIB_PATH + ".%d.tmp" % os.getpid()
-    extra = os.environ.get("TLB_NVCC_EXTRA", "").split()  # experiments only (e.g. -DTLB_EXP=1)
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", _INCLUDE, "-o", tmp] + \
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", _INCLUDE, "-o", tmp] + \
           [os.path.join(_CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB_PATH)
@@ -95,8 +96,21 @@ def load_library():
     lib.tlb_fields_host.argtypes = [vp, dp, dp, dp, dp]
     lib.tlb_observables.argtypes = [vp, dp]
     lib.tlb_observables_host.argtypes = [vp, dp]
-    lib.tlb_x_average.argtypes = [vp, dp]
-    lib.tlb_x_average_host.argtypes = [vp, dp]
+    for name in ("tlb_x_average", "tlb_x_average_host", "tlb_stress_xy", "tlb_stress_xy_host", "tlb_x_average_stress",
+                 "tlb_x_average_stress_host", "tlb_observable_sums"):
+        getattr(lib, name).argtypes = [vp, dp]
+    lib.tlb_observables_from_sums.argtypes = [vp, dp, dp]
+    lib.tlb_slab_workspace_bytes.argtypes = [i32, i32, i32, i32, pp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.tlb_create_slab.argtypes = [i32, i32, i32, i32, pp, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+    lib.tlb_slab_layout.argtypes = [vp, ctypes.POINTER(ctypes.c_int32)]
+    lib.tlb_halo_bytes.argtypes = [vp, ctypes.POINTER(ctypes.c_size_t)]
+    lib.tlb_seg_rows.argtypes = [vp]
+    for name in ("tlb_slab_step_edges", "tlb_slab_step_interior", "tlb_slab_step_finish"):
+        getattr(lib, name).argtypes = [vp]
+    lib.tlb_halo_pack.argtypes = [vp, i32, dp]
+    lib.tlb_halo_unpack.argtypes = [vp, i32, dp]
+    lib.tlb_droplets.argtypes = [vp, ctypes.c_double, dp, i32, dp, dp]
+    lib.tlb_droplets_host.argtypes = [vp, ctypes.c_double, dp, i32, dp, dp]
     lib.tlb_launch_count.argtypes = [vp]
     lib.tlb_launch_count.restype = i64
     lib.tlb_error_string.argtypes = [i32]
@@ -127,17 +141,23 @@ class TLB:
     """One lattice on one GPU.  Methods mirror the C calls; tensors are torch CUDA float64 (device
     variants) or CPU float64 (the *_host variants; pin them for asynchronous copies)."""
 
-    def __init__(self, nx, ny, params=None, device="cuda:0", stream=None, **overrides):
+    def __init__(self, nx, ny, params=None, device="cuda:0", stream=None, slab=None, **overrides):
+        """slab = (y0, y1): a y-slab handle for rows [y0, y1) of the nx x ny lattice (tlb_create_slab); self.ny is
+        then the number of local rows (owned + halo) and self.ny_global the lattice's."""
         import torch
         self.torch = torch
         self.lib = load_library()
-        self.nx, self.ny = int(nx), int(ny)
+        self.nx, self.ny_global = int(nx), int(ny)
         self.params = params if params is not None else default_params(**overrides)
         if params is not None:
             for k, v in overrides.items():
                 setattr(self.params, k, v)
         nbytes = ctypes.c_size_t()
-        self._chk(self.lib.tlb_workspace_bytes(self.nx, self.ny, ctypes.byref(self.params), ctypes.byref(nbytes)))
+        if slab is None:
+            self._chk(self.lib.tlb_workspace_bytes(self.nx, self.ny_global, ctypes.byref(self.params), ctypes.byref(nbytes)))
+        else:
+            self._chk(self.lib.tlb_slab_workspace_bytes(self.nx, self.ny_global, int(slab[0]), int(slab[1]),
+                                                        ctypes.byref(self.params), ctypes.byref(nbytes)))
         if not torch.cuda.is_available():
             raise TLBError(TLB_ECUDA, "no CUDA device; there is no CPU fallback")
         self.device = torch.device(device)
@@ -147,9 +167,17 @@ class TLB:
         base = (self.workspace.data_ptr() + 255) & ~255
         h = ctypes.c_void_p()
         self.h = None
-        self._chk(self.lib.tlb_create(self.nx, self.ny, ctypes.byref(self.params), base, nbytes.value,
-                                      self.stream.cuda_stream, ctypes.byref(h)))
+        if slab is None:
+            self._chk(self.lib.tlb_create(self.nx, self.ny_global, ctypes.byref(self.params), base, nbytes.value,
+                                          self.stream.cuda_stream, ctypes.byref(h)))
+        else:
+            self._chk(self.lib.tlb_create_slab(self.nx, self.ny_global, int(slab[0]), int(slab[1]),
+                                               ctypes.byref(self.params), base, nbytes.value,
+                                               self.stream.cuda_stream, ctypes.byref(h)))
         self.h = h
+        lay = (ctypes.c_int32 * 6)()
+        self._chk(self.lib.tlb_slab_layout(self.h, lay))
+        self.ny, self.own0, self.own1, self.y_off, self.halo_lo, self.halo_hi = (int(v) for v in lay)
 
     def _chk(self, rc):
         if rc != TLB_OK:
@@ -174,7 +202,10 @@ class TLB:
         dtype = dtype or torch.float64
         t = torch.as_tensor(t)
         if t.device != self.device or t.dtype != dtype or not t.is_contiguous():
-            t = t.to(device=self.device, dtype=dtype).contiguous()
+            # convert on the handle's stream: the kernels that read the temporary are enqueued there, so neither
+            # the copy nor the caching allocator's reuse of the block can race with them
+            with torch.cuda.stream(self.stream):
+                t = t.to(device=self.device, dtype=dtype).contiguous()
         assert tuple(t.shape) == tuple(shape), (tuple(t.shape), shape)
         return t
 
@@ -270,6 +301,89 @@ class TLB:
     def observables_device(self, out4):
         self._chk(self.lib.tlb_observables(self.h, out4.data_ptr()))
         return out4
+
+    def observable_sums(self, out6=None):
+        """sums6 (device tensor): this handle's share of the six sums behind the observables."""
+        out6 = self._new(6) if out6 is None else out6
+        self._chk(self.lib.tlb_observable_sums(self.h, out6.data_ptr()))
+        return out6
+
+    def observables_from_sums(self, sums6):
+        """dict(mass_A, mass_B, E, Nu) from (all-reduced) sums6 (device tensor)."""
+        out = self._new(4)
+        self._chk(self.lib.tlb_observables_from_sums(self.h, sums6.data_ptr(), out.data_ptr()))
+        v = out.cpu().tolist()
+        return dict(mass_A=v[0], mass_B=v[1], E=v[2], Nu=v[3])
+
+    def stress_xy(self):
+        """P_xy [ny][nx] (device tensor), reading R21."""
+        out = self._new(self.ny, self.nx)
+        self._chk(self.lib.tlb_stress_xy(self.h, out.data_ptr()))
+        return out
+
+    def stress_xy_host(self, out=None):
+        if out is None:
+            out = self.torch.empty((self.ny, self.nx), dtype=self.torch.float64)
+        out = self._host(out, (self.ny, self.nx))
+        self._chk(self.lib.tlb_stress_xy_host(self.h, out.data_ptr()))
+        return out
+
+    def x_average_stress(self):
+        """Pxy_av[ny]: x-average of P_xy over the fluid sites of each row (device tensor)."""
+        out = self._new(self.ny)
+        self._chk(self.lib.tlb_x_average_stress(self.h, out.data_ptr()))
+        return out
+
+    def x_average_stress_host(self, out=None):
+        if out is None:
+            out = self.torch.empty(self.ny, dtype=self.torch.float64)
+        out = self._host(out, (self.ny,))
+        self._chk(self.lib.tlb_x_average_stress_host(self.h, out.data_ptr()))
+        return out
+
+    def droplets(self, B_th, max_droplets, want_labels=True):
+        """(labels [ny][nx] int32 or None, n_droplets, stats [n][4]) as device tensors / int (section 2.4, R22)."""
+        torch = self.torch
+        labels = torch.empty((self.ny, self.nx), dtype=torch.int32, device=self.device) if want_labels else None
+        n = torch.zeros(1, dtype=torch.int32, device=self.device)
+        stats = torch.zeros((max(1, max_droplets), 4), dtype=torch.float64, device=self.device)
+        self._chk(self.lib.tlb_droplets(self.h, float(B_th), _ptr(labels), int(max_droplets), n.data_ptr(), stats.data_ptr()))
+        k = int(n.item())
+        return labels, k, stats[:min(k, max_droplets)]
+
+    def droplets_host(self, B_th, max_droplets, want_labels=True):
+        torch = self.torch
+        labels = torch.empty((self.ny, self.nx), dtype=torch.int32) if want_labels else None
+        n = torch.zeros(1, dtype=torch.int32)
+        stats = torch.zeros((max(1, max_droplets), 4), dtype=torch.float64)
+        self._chk(self.lib.tlb_droplets_host(self.h, float(B_th), _ptr(labels), int(max_droplets), n.data_ptr(), stats.data_ptr()))
+        k = int(n.item())
+        return labels, k, stats[:min(k, max_droplets)]
+
+    def seg_rows(self):
+        return int(self.lib.tlb_seg_rows(self.h))
+
+    # ---- y-slab stepping (tlb.h "Y-SLABS") ---------------------------------------------------
+    def halo_buffer(self):
+        """A device buffer of tlb_halo_bytes (one packed face)."""
+        nb = ctypes.c_size_t()
+        self._chk(self.lib.tlb_halo_bytes(self.h, ctypes.byref(nb)))
+        return self.torch.empty(nb.value, dtype=self.torch.uint8, device=self.device)
+
+    def slab_step_edges(self):
+        self._chk(self.lib.tlb_slab_step_edges(self.h))
+
+    def slab_step_interior(self):
+        self._chk(self.lib.tlb_slab_step_interior(self.h))
+
+    def slab_step_finish(self):
+        self._chk(self.lib.tlb_slab_step_finish(self.h))
+
+    def halo_pack(self, face, buf):
+        self._chk(self.lib.tlb_halo_pack(self.h, int(face), buf.data_ptr()))
+
+    def halo_unpack(self, face, buf):
+        self._chk(self.lib.tlb_halo_unpack(self.h, int(face), buf.data_ptr()))
 
     def launch_count(self):
         return int(self.lib.tlb_launch_count(self.h))

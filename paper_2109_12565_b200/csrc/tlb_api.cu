@@ -14,19 +14,26 @@ struct tlb_handle {
   Dev d;
   tlb_params p;
   cudaStream_t st;
+  int device;         // CUDA device of the workspace; every entry point runs with it current
   void* S[2];         // population buffers (pull form), 27 planes each, double or float (pop_precision)
   double* stage;      // [27][ny][nx] doubles for the *_host population calls when the buffers are float
   double* fld[5];     // rho_A, rho_B, u_x, u_y, T scratch planes
   uint8_t* solid;
-  uint8_t* solidp;     // padded copy for the fused kernel
+  uint8_t* solidp;    // padded copy for the fused kernel
   int* sites;         // boundary work list
   int* count;
-  double* partials;
+  double* partials;   // [obs_ctas][6] partial sums of the observables
+  double* sums6;
   double* out4;
+  int* n_drop;
   double* centres;
   int cur;            // S[cur] holds the current state
   int n_sites;
   int seg_rows;
+  int obs_ctas;
+  int halo_lo, halo_hi;  // y-slab: halo rows beyond the low / high face (0 at a wall or for a whole lattice)
+  bool slab;
+  bool step_open;     // between tlb_slab_step_edges and tlb_slab_step_finish
   bool has_state;
   cudaError_t err;
   int64_t launches;
@@ -41,11 +48,36 @@ namespace {
 
 size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
-struct Layout {
-  size_t S0, S1, stage, fld, solid, solidp, sites, count, partials, out4, centres, total;
+struct Geometry {  // local lattice of a handle
+  int ny, y_off, own0, own1, halo_lo, halo_hi;
 };
 
-Layout make_layout(int nx, int ny, const tlb_params* p) {
+// Whole lattice: rows [0, ny_glob).  Slab: owned rows [y0, y1) plus kHalo imported rows beyond every face that is
+// not a flat wall (a face of the whole lattice is one unless the lattice is periodic in y).
+bool make_geometry(int ny_glob, int y0, int y1, bool slab, bool periodic, Geometry* g) {
+  if (!slab) { *g = Geometry{ny_glob, 0, 0, ny_glob, 0, 0}; return true; }
+  if (y0 < 0 || y1 > ny_glob || y1 <= y0) return false;
+  g->halo_lo = (y0 == 0 && !periodic) ? 0 : kHalo;
+  g->halo_hi = (y1 == ny_glob && !periodic) ? 0 : kHalo;
+  if ((g->halo_lo || g->halo_hi) && y1 - y0 < kHalo) return false;  // a neighbour imports kHalo of these rows
+  g->ny = (y1 - y0) + g->halo_lo + g->halo_hi;
+  g->y_off = y0 - g->halo_lo;
+  g->own0 = g->halo_lo;
+  g->own1 = g->halo_lo + (y1 - y0);
+  return true;
+}
+
+int obs_cta_count(int nx, int own_rows) {
+  const int seg = default_seg_rows(nx, own_rows);
+  return ((nx + kW - 1) / kW) * ((own_rows + seg - 1) / seg);
+}
+
+struct Layout {
+  size_t S0, S1, stage, fld, solid, solidp, sites, count, partials, sums6, out4, n_drop, centres, total;
+};
+
+Layout make_layout(int nx, const Geometry& g, const tlb_params* p) {
+  const int ny = g.ny;
   const size_t n = (size_t)nx * ny, px = (size_t)padded_pitch(nx), plane = px * (ny + 2);
   Layout L;
   size_t o = 0;
@@ -59,8 +91,10 @@ Layout make_layout(int nx, int ny, const tlb_params* p) {
   L.solidp = o; o = align_up(o + px * ny);
   L.sites = o; o = align_up(o + n * sizeof(int));
   L.count = o; o = align_up(o + sizeof(int));
-  L.partials = o; o = align_up(o + (size_t)kObsBlocks * 8 * sizeof(double));
+  L.partials = o; o = align_up(o + (size_t)obs_cta_count(nx, g.own1 - g.own0) * 6 * sizeof(double));
+  L.sums6 = o; o = align_up(o + 6 * sizeof(double));
   L.out4 = o; o = align_up(o + 4 * sizeof(double));
+  L.n_drop = o; o = align_up(o + sizeof(int));
   L.centres = o; o = align_up(o + 2 * sizeof(double) * (size_t)(p->n_droplets > 0 ? p->n_droplets : 1));
   L.total = o;
   return L;
@@ -68,8 +102,8 @@ Layout make_layout(int nx, int ny, const tlb_params* p) {
 
 bool params_ok(int nx, int ny, const tlb_params* p) {
   if (nx < 1 || ny < 1 || !p) return false;
-  if ((long long)padded_pitch(nx) * (ny + 2) * 27 >= (1ll << 40)) return false;
-  if ((long long)nx * ny >= (1ll << 31)) return false;
+  if ((long long)padded_pitch(nx) * (ny + 2 + 2 * kHalo) * 27 >= (1ll << 40)) return false;
+  if ((long long)nx * (ny + 2 * kHalo) >= (1ll << 31)) return false;
   if (!(p->tau > 0.5) || !(p->tau_g > 0.5) || !(p->rho0 > 0.0)) return false;
   if (p->pop_precision != 64 && p->pop_precision != 32 && p->pop_precision != 0) return false;
   if (p->n_droplets < 0 || p->post_w < 0 || p->post_h < 0 || p->post_period < 0) return false;
@@ -79,6 +113,9 @@ bool params_ok(int nx, int ny, const tlb_params* p) {
   return true;
 }
 
+// Errors.  The handle keeps the first error of its OWN calls (sticky).  cudaGetLastError() is only read right
+// after the handle's own launches (check()), and an error another library left pending on this thread is neither
+// consumed nor adopted: enter() reports it without touching the handle.
 int check(tlb_handle* h) {
   if (h->err == cudaSuccess) h->err = cudaGetLastError();
   return h->err == cudaSuccess ? TLB_OK : TLB_ECUDA;
@@ -88,11 +125,34 @@ int cu(tlb_handle* h, cudaError_t e) {
   return h->err == cudaSuccess ? TLB_OK : TLB_ECUDA;
 }
 
+// Makes the handle's device current for the duration of an entry point and restores the caller's.
+struct Enter {
+  int prev = -1, rc = TLB_OK;
+  bool switched = false;
+  explicit Enter(tlb_handle* h) {
+    if (h->err != cudaSuccess) { rc = TLB_ECUDA; return; }
+    if (cudaGetDevice(&prev) != cudaSuccess) { rc = TLB_ECUDA; return; }
+    if (prev != h->device) {
+      if (cudaSetDevice(h->device) != cudaSuccess) { rc = TLB_ECUDA; return; }
+      switched = true;
+    }
+    if (cudaPeekAtLastError() != cudaSuccess) rc = TLB_ECUDA;  // somebody else's pending error: not ours to consume
+  }
+  ~Enter() { if (switched) cudaSetDevice(prev); }
+};
+#define TLB_ENTER(h)         \
+  Enter enter_guard(h);      \
+  if (enter_guard.rc != TLB_OK) return enter_guard.rc
+
 constexpr int kGraphSteps = 16;
 
 void drop_graphs(tlb_handle* h) {
   for (int k = 0; k < 2; k++)
     if (h->gexec[k]) { cudaGraphExecDestroy(h->gexec[k]); h->gexec[k] = nullptr; }
+}
+
+int launch_step(tlb_handle* h, const void* in, void* out, int ya, int yb, cudaStream_t st) {
+  return launch_fused(h->d, 0, in, out, h->seg_rows, ya, yb, FusedOut{}, st);
 }
 
 // Capture kGraphSteps steps starting from buffer parity `cur` (kernel arguments are baked in: the
@@ -109,7 +169,7 @@ bool ensure_graph(tlb_handle* h, int cur) {
   int64_t n = 0;
   int c = cur;
   for (int t = 0; t < kGraphSteps; t++) {
-    n += launch_step(h->d, h->S[c], h->S[1 - c], h->seg_rows, h->cap_stream);
+    n += launch_step(h, h->S[c], h->S[1 - c], h->d.own0, h->d.own1, h->cap_stream);
     n += launch_boundary(h->d, h->S[1 - c], h->sites, h->n_sites, h->cap_stream);
     c = 1 - c;
   }
@@ -129,6 +189,7 @@ bool ensure_graph(tlb_handle* h, int cur) {
 
 // After the mask changed: rebuild the boundary work list (count comes back to size the launch).
 int rebuild_links(tlb_handle* h) {
+  cu(h, cudaMemsetAsync(h->count, 0, sizeof(int), h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);
   int c = 0;
   cu(h, cudaMemcpyAsync(&c, h->count, sizeof(int), cudaMemcpyDeviceToHost, h->st));
@@ -136,6 +197,7 @@ int rebuild_links(tlb_handle* h) {
   h->n_sites = c;
   drop_graphs(h);
   h->has_state = false;
+  h->step_open = false;
   return check(h);
 }
 
@@ -144,6 +206,7 @@ int rebuild_links(tlb_handle* h) {
 int after_state_set(tlb_handle* h) {
   if (!h->d.thermal) h->launches += launch_copy_g(h->d, h->S[h->cur], h->S[1 - h->cur], h->st);
   h->has_state = true;
+  h->step_open = false;
   return check(h);
 }
 
@@ -224,26 +287,47 @@ int tlb_default_params(tlb_params* p) {
   return TLB_OK;
 }
 
-int tlb_workspace_bytes(int nx, int ny, const tlb_params* p, size_t* bytes) {
-  if (!bytes || !params_ok(nx, ny, p)) return TLB_EINVAL;
-  *bytes = make_layout(nx, ny, p).total;
+static int workspace_bytes_common(int nx, int ny_glob, int y0, int y1, bool slab, const tlb_params* p, size_t* bytes) {
+  Geometry g;
+  if (!bytes || !params_ok(nx, ny_glob, p) || !make_geometry(ny_glob, y0, y1, slab, p->periodic_y != 0, &g)) return TLB_EINVAL;
+  *bytes = make_layout(nx, g, p).total;
   return TLB_OK;
 }
 
-int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t workspace_bytes, void* stream,
-               tlb_handle** out) {
+int tlb_workspace_bytes(int nx, int ny, const tlb_params* p, size_t* bytes) {
+  return workspace_bytes_common(nx, ny, 0, ny, false, p, bytes);
+}
+
+int tlb_slab_workspace_bytes(int nx, int ny, int y0, int y1, const tlb_params* p, size_t* bytes) {
+  return workspace_bytes_common(nx, ny, y0, y1, true, p, bytes);
+}
+
+static int create_common(int nx, int ny_glob, int y0, int y1, bool slab, const tlb_params* p, void* workspace,
+                         size_t workspace_bytes, void* stream, tlb_handle** out) {
   if (!out) return TLB_EINVAL;
   *out = nullptr;
-  if (!params_ok(nx, ny, p) || !workspace || ((uintptr_t)workspace & 255)) return TLB_EINVAL;
-  const Layout L = make_layout(nx, ny, p);
+  Geometry g;
+  if (!params_ok(nx, ny_glob, p) || !workspace || ((uintptr_t)workspace & 255)) return TLB_EINVAL;
+  if (!make_geometry(ny_glob, y0, y1, slab, p->periodic_y != 0, &g)) return TLB_EINVAL;
+  const Layout L = make_layout(nx, g, p);
   if (workspace_bytes < L.total) return TLB_EINVAL;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
     cudaGetLastError();
     return TLB_ECUDA;  // no CPU fallback
   }
+  cudaPointerAttributes attr;
+  if (cudaPointerGetAttributes(&attr, workspace) != cudaSuccess || attr.type != cudaMemoryTypeDevice) {
+    cudaGetLastError();
+    return TLB_EINVAL;  // `workspace` is not device memory
+  }
   tlb_handle* h = new (std::nothrow) tlb_handle();
   if (!h) return TLB_EINVAL;
+  h->device = attr.device;
+  h->err = cudaSuccess;
+  Enter guard(h);
+  if (guard.rc != TLB_OK) { delete h; return guard.rc; }
+  const int ny = g.ny;
   char* w = static_cast<char*>(workspace);
   h->p = *p;
   h->st = static_cast<cudaStream_t>(stream);
@@ -256,10 +340,18 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   h->sites = reinterpret_cast<int*>(w + L.sites);
   h->count = reinterpret_cast<int*>(w + L.count);
   h->partials = reinterpret_cast<double*>(w + L.partials);
+  h->sums6 = reinterpret_cast<double*>(w + L.sums6);
   h->out4 = reinterpret_cast<double*>(w + L.out4);
+  h->n_drop = reinterpret_cast<int*>(w + L.n_drop);
   h->centres = reinterpret_cast<double*>(w + L.centres);
+  h->slab = slab; h->halo_lo = g.halo_lo; h->halo_hi = g.halo_hi; h->step_open = false;
   Dev& d = h->d;
-  d.nx = nx; d.ny = ny; d.periodic_y = p->periodic_y ? 1 : 0; d.thermal = p->thermal ? 1 : 0;
+  d.nx = nx; d.ny = ny; d.thermal = p->thermal ? 1 : 0;
+  d.y_off = g.y_off; d.ny_glob = ny_glob; d.per_glob = p->periodic_y ? 1 : 0;
+  d.own0 = g.own0; d.own1 = g.own1;
+  d.periodic_y = (!slab && p->periodic_y) ? 1 : 0;  // a slab is never periodic by itself: its faces import halo rows
+  d.wall_lo = (!p->periodic_y && g.halo_lo == 0) ? 1 : 0;
+  d.wall_hi = (!p->periodic_y && g.halo_hi == 0) ? 1 : 0;
   d.px = padded_pitch(nx);
   d.prec = p->pop_precision == 32 ? 32 : 64;
   d.plane = (long long)d.px * (ny + 2);
@@ -274,14 +366,12 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   d.u_wall_bottom = p->u_wall_bottom; d.u_wall_top = p->u_wall_top;
   d.solid = h->solid;
   d.solidp = h->solidp;
-  h->cur = 0; h->n_sites = 0; h->has_state = false; h->err = cudaSuccess; h->launches = 0;
-  int seg = default_seg_rows(nx, ny);
-  if (const char* e = std::getenv("TLB_SEG_ROWS")) { const int v = std::atoi(e); if (v > 0) seg = v; }
-  if (seg > ny) seg = ny;
-  h->seg_rows = seg;
+  h->cur = 0; h->n_sites = 0; h->has_state = false; h->launches = 0;
+  h->seg_rows = default_seg_rows(nx, g.own1 - g.own0);
+  h->obs_ctas = obs_cta_count(nx, g.own1 - g.own0);
   h->gexec[0] = h->gexec[1] = nullptr;
   h->cap_stream = nullptr;
-  h->use_graph = std::getenv("TLB_NO_GRAPH") == nullptr;
+  h->use_graph = !(slab && (g.halo_lo || g.halo_hi));  // a slab's step is driven call by call (halo exchange in between)
   if (h->use_graph && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
     cudaGetLastError();
     h->cap_stream = nullptr;
@@ -289,6 +379,7 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   }
   if (configure_kernels() != 0) { cudaGetLastError(); tlb_destroy(h); return TLB_ECUDA; }
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
+  cu(h, cudaMemsetAsync(h->count, 0, sizeof(int), h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field
   cu(h, cudaMemsetAsync(h->S[0], 0, 27 * (size_t)d.px * (ny + 2) * (d.prec == 32 ? sizeof(float) : sizeof(double)), h->st));
   cu(h, cudaMemsetAsync(h->S[1], 0, 27 * (size_t)d.px * (ny + 2) * (d.prec == 32 ? sizeof(float) : sizeof(double)), h->st));
@@ -297,26 +388,56 @@ int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t work
   return TLB_OK;
 }
 
+int tlb_create(int nx, int ny, const tlb_params* p, void* workspace, size_t workspace_bytes, void* stream,
+               tlb_handle** out) {
+  return create_common(nx, ny, 0, ny, false, p, workspace, workspace_bytes, stream, out);
+}
+
+int tlb_create_slab(int nx, int ny, int y0, int y1, const tlb_params* p, void* workspace, size_t workspace_bytes,
+                    void* stream, tlb_handle** out) {
+  return create_common(nx, ny, y0, y1, true, p, workspace, workspace_bytes, stream, out);
+}
+
 int tlb_destroy(tlb_handle* h) {
   if (!h) return TLB_EINVAL;
+  int prev = -1;
+  cudaGetDevice(&prev);
+  if (prev != h->device) cudaSetDevice(h->device);
   cudaStreamSynchronize(h->st);
   drop_graphs(h);
   if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  if (prev >= 0 && prev != h->device) cudaSetDevice(prev);
   delete h;
   return TLB_OK;
 }
 
+int tlb_slab_layout(const tlb_handle* h, int32_t out6[6]) {
+  if (!h || !out6) return TLB_EINVAL;
+  out6[0] = h->d.ny; out6[1] = h->d.own0; out6[2] = h->d.own1; out6[3] = h->d.y_off; out6[4] = h->halo_lo; out6[5] = h->halo_hi;
+  return TLB_OK;
+}
+
+int tlb_halo_bytes(const tlb_handle* h, size_t* bytes) {
+  if (!h || !bytes) return TLB_EINVAL;
+  *bytes = 27 * (size_t)kHalo * h->d.px * (h->d.prec == 32 ? sizeof(float) : sizeof(double));
+  return TLB_OK;
+}
+
+int tlb_seg_rows(const tlb_handle* h) { return h ? h->seg_rows : TLB_EINVAL; }
+
 int tlb_init(tlb_handle* h, uint64_t seed) {
   if (!h) return TLB_EINVAL;
+  TLB_ENTER(h);
   std::vector<double> c;
-  if (!place_droplets(h->d.nx, h->d.ny, seed, h->p, c)) return TLB_EPLACEMENT;
+  if (!place_droplets(h->d.nx, h->d.ny_glob, seed, h->p, c)) return TLB_EPLACEMENT;
   const int n = (int)(c.size() / 2);
   if (n > 0) {
     cu(h, cudaMemcpyAsync(h->centres, c.data(), c.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
     cu(h, cudaStreamSynchronize(h->st));  // `c` is pageable and dies with this frame
   }
-  h->launches += launch_init(h->d, h->p, seed, h->centres, n, reinterpret_cast<uint8_t*>(h->fld[2]), h->solid,
-                             h->fld[0], h->fld[1], h->fld[4], h->st);
+  uint8_t* inside = reinterpret_cast<uint8_t*>(h->fld[2]);
+  cu(h, cudaMemsetAsync(inside, 0, (size_t)h->d.nx * h->d.ny, h->st));
+  h->launches += launch_init(h->d, h->p, seed, h->centres, n, inside, h->solid, h->fld[0], h->fld[1], h->fld[4], h->st);
   int rc = rebuild_links(h);
   if (rc != TLB_OK) return rc;
   h->launches += launch_set_fields(h->d, h->fld[0], h->fld[1], h->fld[4], h->S[h->cur], h->st);
@@ -325,24 +446,28 @@ int tlb_init(tlb_handle* h, uint64_t seed) {
 
 int tlb_set_solid(tlb_handle* h, const uint8_t* solid) {
   if (!h || !solid) return TLB_EINVAL;
+  TLB_ENTER(h);
   cu(h, cudaMemcpyAsync(h->solid, solid, (size_t)h->d.nx * h->d.ny, cudaMemcpyDeviceToDevice, h->st));
   return rebuild_links(h);
 }
 
 int tlb_set_solid_host(tlb_handle* h, const uint8_t* solid) {
   if (!h || !solid) return TLB_EINVAL;
+  TLB_ENTER(h);
   cu(h, cudaMemcpyAsync(h->solid, solid, (size_t)h->d.nx * h->d.ny, cudaMemcpyHostToDevice, h->st));
   return rebuild_links(h);
 }
 
 int tlb_set_fields(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T) {
   if (!h || !rho_A || !rho_B || !T) return TLB_EINVAL;
+  TLB_ENTER(h);
   h->launches += launch_set_fields(h->d, rho_A, rho_B, T, h->S[h->cur], h->st);
   return after_state_set(h);
 }
 
 int tlb_set_fields_host(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T) {
   if (!h || !rho_A || !rho_B || !T) return TLB_EINVAL;
+  TLB_ENTER(h);
   const size_t b = (size_t)h->d.nx * h->d.ny * sizeof(double);
   cu(h, cudaMemcpyAsync(h->fld[0], rho_A, b, cudaMemcpyHostToDevice, h->st));
   cu(h, cudaMemcpyAsync(h->fld[1], rho_B, b, cudaMemcpyHostToDevice, h->st));
@@ -355,6 +480,7 @@ int tlb_set_fields_host(tlb_handle* h, const double* rho_A, const double* rho_B,
 
 int tlb_set_populations(tlb_handle* h, const double* fA, const double* fB, const double* g) {
   if (!h || !fA || !fB || !g) return TLB_EINVAL;
+  TLB_ENTER(h);
   h->launches += launch_scatter(h->d, fA, fB, g, h->S[h->cur], h->st);
   return after_state_set(h);
 }
@@ -362,6 +488,7 @@ int tlb_set_populations(tlb_handle* h, const double* fA, const double* fB, const
 int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g) {
   if (!h) return TLB_EINVAL;
   if (!h->has_state) return TLB_ESTATE;
+  TLB_ENTER(h);
   h->launches += launch_gather(h->d, h->S[h->cur], fA, fB, g, h->st);
   return check(h);
 }
@@ -370,6 +497,7 @@ int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g) {
 // next step anyway; its g planes are restored when thermal = 0).
 int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, const double* g) {
   if (!h || !fA || !fB || !g) return TLB_EINVAL;
+  TLB_ENTER(h);
   const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
   double* stage = h->stage ? h->stage : static_cast<double*>(h->S[1 - h->cur]);
   cu(h, cudaMemcpyAsync(stage, fA, n9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
@@ -386,6 +514,7 @@ int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, 
 int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g) {
   if (!h || !fA || !fB || !g) return TLB_EINVAL;
   if (!h->has_state) return TLB_ESTATE;
+  TLB_ENTER(h);
   const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
   double* stage = h->stage ? h->stage : static_cast<double*>(h->S[1 - h->cur]);
   h->launches += launch_gather(h->d, h->S[h->cur], stage, stage + n9, stage + 2 * n9, h->st);
@@ -399,8 +528,12 @@ int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g) {
 
 int tlb_step(tlb_handle* h, int64_t n) {
   if (!h || n < 0) return TLB_EINVAL;
+  if (h->halo_lo || h->halo_hi) return TLB_EINVAL;  // a slab with halo rows steps through the tlb_slab_step_* calls
   if (!h->has_state) return TLB_ESTATE;
-  if (h->err != cudaSuccess) return TLB_ECUDA;
+  TLB_ENTER(h);
+  // the graphs of both buffer parities are captured on the first call, before anything is enqueued, so that a
+  // caller timing a later call never times cudaGraphInstantiate
+  if (n > 0 && h->use_graph) { ensure_graph(h, 0); ensure_graph(h, 1); }
   int64_t t = 0;
   // whole blocks of kGraphSteps steps replay a captured graph (one launch instead of 2 * kGraphSteps)
   while (n - t >= kGraphSteps && ensure_graph(h, h->cur)) {
@@ -411,17 +544,74 @@ int tlb_step(tlb_handle* h, int64_t n) {
   for (; t < n; t++) {
     void* in = h->S[h->cur];
     void* out = h->S[1 - h->cur];
-    h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);
+    h->launches += launch_step(h, in, out, h->d.own0, h->d.own1, h->st);
     h->launches += launch_boundary(h->d, out, h->sites, h->n_sites, h->st);
     h->cur = 1 - h->cur;
   }
   return check(h);
 }
 
+// ---- y-slab stepping: edges -> (pack, exchange, unpack by the caller) -> interior -> finish ----
+static void edge_rows(const tlb_handle* h, int* lo_end, int* hi_beg) {
+  const int a = h->d.own0, b = h->d.own1;
+  *lo_end = h->halo_lo ? (a + kHalo < b ? a + kHalo : b) : a;
+  const int hb = h->halo_hi ? b - kHalo : b;
+  *hi_beg = hb > *lo_end ? hb : *lo_end;
+}
+
+int tlb_slab_step_edges(tlb_handle* h) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  int lo_end, hi_beg;
+  edge_rows(h, &lo_end, &hi_beg);
+  h->launches += launch_step(h, h->S[h->cur], h->S[1 - h->cur], h->d.own0, lo_end, h->st);
+  h->launches += launch_step(h, h->S[h->cur], h->S[1 - h->cur], hi_beg, h->d.own1, h->st);
+  h->step_open = true;
+  return check(h);
+}
+
+int tlb_slab_step_interior(tlb_handle* h) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state || !h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  int lo_end, hi_beg;
+  edge_rows(h, &lo_end, &hi_beg);
+  h->launches += launch_step(h, h->S[h->cur], h->S[1 - h->cur], lo_end, hi_beg, h->st);
+  return check(h);
+}
+
+int tlb_slab_step_finish(tlb_handle* h) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state || !h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  h->launches += launch_boundary(h->d, h->S[1 - h->cur], h->sites, h->n_sites, h->st);
+  h->cur = 1 - h->cur;
+  h->step_open = false;
+  return check(h);
+}
+
+int tlb_halo_pack(tlb_handle* h, int face, void* buf) {
+  if (!h || !buf || face < 0 || face > 1 || !(face ? h->halo_hi : h->halo_lo)) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  TLB_ENTER(h);
+  h->launches += launch_halo_pack(h->d, h->S[h->step_open ? 1 - h->cur : h->cur], face, buf, h->st);
+  return check(h);
+}
+
+int tlb_halo_unpack(tlb_handle* h, int face, const void* buf) {
+  if (!h || !buf || face < 0 || face > 1 || !(face ? h->halo_hi : h->halo_lo)) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  TLB_ENTER(h);
+  h->launches += launch_halo_unpack(h->d, h->S[h->step_open ? 1 - h->cur : h->cur], face, buf, h->st);
+  return check(h);
+}
+
 int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundary_ms) {
   if (!h || n < 1 || n > 4096 || !fused_ms || !boundary_ms) return TLB_EINVAL;
+  if (h->halo_lo || h->halo_hi) return TLB_EINVAL;
   if (!h->has_state) return TLB_ESTATE;
-  if (h->err != cudaSuccess) return TLB_ECUDA;
+  TLB_ENTER(h);
   // Both kernels are idempotent on fixed inputs (the fused kernel reads S[cur] and writes S[1-cur]; the
   // boundary kernel reads fluid nodes and writes solid / ghost nodes), so each is launched n times back
   // to back between two events and the state advances by exactly one step.
@@ -430,7 +620,7 @@ int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundar
   void* in = h->S[h->cur];
   void* out = h->S[1 - h->cur];
   cu(h, cudaEventRecord(ev[0], h->st));
-  for (int64_t t = 0; t < n; t++) h->launches += launch_step(h->d, in, out, h->seg_rows, h->st);
+  for (int64_t t = 0; t < n; t++) h->launches += launch_step(h, in, out, h->d.own0, h->d.own1, h->st);
   cu(h, cudaEventRecord(ev[1], h->st));
   for (int64_t t = 0; t < n; t++) h->launches += launch_boundary(h->d, out, h->sites, h->n_sites, h->st);
   cu(h, cudaEventRecord(ev[2], h->st));
@@ -447,22 +637,33 @@ int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundar
   return check(h);
 }
 
-static int fields_to_scratch(tlb_handle* h) {
-  h->launches += launch_fields(h->d, h->S[h->cur], h->fld[0], h->fld[1], h->fld[2], h->fld[3], h->fld[4], h->st);
+// rows the non-stepping modes of the fused kernel sweep: the owned ones
+static int fused_mode(tlb_handle* h, int mode, const FusedOut& out) {
+  const int seg = default_seg_rows(h->d.nx, h->d.own1 - h->d.own0);
+  h->launches += launch_fused(h->d, mode, h->S[h->cur], nullptr, seg, h->d.own0, h->d.own1, out, h->st);
   return check(h);
+}
+
+static int fields_to_scratch(tlb_handle* h) {
+  FusedOut o{};
+  o.rhoA = h->fld[0]; o.rhoB = h->fld[1]; o.ux = h->fld[2]; o.uy = h->fld[3]; o.T = h->fld[4];
+  return fused_mode(h, 1, o);
 }
 
 int tlb_fields(tlb_handle* h, double* rho_A, double* rho_B, double* u, double* T) {
   if (!h) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
   const size_t n = (size_t)h->d.nx * h->d.ny;
-  h->launches += launch_fields(h->d, h->S[h->cur], rho_A, rho_B, u, u ? u + n : nullptr, T, h->st);
-  return check(h);
+  FusedOut o{};
+  o.rhoA = rho_A; o.rhoB = rho_B; o.ux = u; o.uy = u ? u + n : nullptr; o.T = T;
+  return fused_mode(h, 1, o);
 }
 
 int tlb_fields_host(tlb_handle* h, double* rho_A, double* rho_B, double* u, double* T) {
   if (!h) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
   const size_t n = (size_t)h->d.nx * h->d.ny, b = n * sizeof(double);
   fields_to_scratch(h);
   if (rho_A) cu(h, cudaMemcpyAsync(rho_A, h->fld[0], b, cudaMemcpyDeviceToHost, h->st));
@@ -473,27 +674,52 @@ int tlb_fields_host(tlb_handle* h, double* rho_A, double* rho_B, double* u, doub
   return check(h);
 }
 
+// one pass: the fused kernel (MODE 3) reduces inside each CTA, a single small kernel combines the CTAs
+static int observable_pass(tlb_handle* h, double* sums6, double* out4) {
+  FusedOut o{};
+  o.partials = h->partials;
+  int rc = fused_mode(h, 3, o);
+  if (rc != TLB_OK) return rc;
+  h->launches += launch_observables_final(h->d, h->partials, h->obs_ctas, sums6, out4, h->st);
+  return check(h);
+}
+
 int tlb_observables(tlb_handle* h, double* out4) {
   if (!h || !out4) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
-  fields_to_scratch(h);
-  h->launches += launch_observables(h->d, h->fld[0], h->fld[1], h->fld[2], h->fld[3], h->fld[4], h->partials,
-                                    kObsBlocks, out4, h->st);
-  return check(h);
+  if (h->halo_lo || h->halo_hi) return TLB_EINVAL;  // a slab holds part of the sums: tlb_observable_sums
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  return observable_pass(h, nullptr, out4);
 }
 
 int tlb_observables_host(tlb_handle* h, double* out4) {
   if (!h || !out4) return TLB_EINVAL;
   int rc = tlb_observables(h, h->out4);
   if (rc != TLB_OK) return rc;
+  TLB_ENTER(h);
   cu(h, cudaMemcpyAsync(out4, h->out4, 4 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
   cu(h, cudaStreamSynchronize(h->st));
   return check(h);
 }
 
+int tlb_observable_sums(tlb_handle* h, double* sums6) {
+  if (!h || !sums6) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  return observable_pass(h, sums6, nullptr);
+}
+
+int tlb_observables_from_sums(tlb_handle* h, const double* sums6, double* out4) {
+  if (!h || !sums6 || !out4) return TLB_EINVAL;
+  TLB_ENTER(h);
+  h->launches += launch_observables_from_sums(h->d, sums6, out4, h->st);
+  return check(h);
+}
+
 int tlb_x_average(tlb_handle* h, double* u_av) {
   if (!h || !u_av) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
   fields_to_scratch(h);
   h->launches += launch_x_average(h->d, h->fld[2], u_av, h->st);
   return check(h);
@@ -501,11 +727,90 @@ int tlb_x_average(tlb_handle* h, double* u_av) {
 
 int tlb_x_average_host(tlb_handle* h, double* u_av) {
   if (!h || !u_av) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
   fields_to_scratch(h);
   // fld[0] (rho_A scratch) is free once the profile has been reduced from fld[2]
   h->launches += launch_x_average(h->d, h->fld[2], h->fld[0], h->st);
   cu(h, cudaMemcpyAsync(u_av, h->fld[0], (size_t)h->d.ny * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
+int tlb_stress_xy(tlb_handle* h, double* P_xy) {
+  if (!h || !P_xy) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  FusedOut o{};
+  o.pxy = P_xy;
+  return fused_mode(h, 2, o);
+}
+
+int tlb_stress_xy_host(tlb_handle* h, double* P_xy) {
+  if (!h || !P_xy) return TLB_EINVAL;
+  int rc = tlb_stress_xy(h, h->fld[0]);
+  if (rc != TLB_OK) return rc;
+  TLB_ENTER(h);
+  cu(h, cudaMemcpyAsync(P_xy, h->fld[0], (size_t)h->d.nx * h->d.ny * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
+int tlb_x_average_stress(tlb_handle* h, double* Pxy_av) {
+  if (!h || !Pxy_av) return TLB_EINVAL;
+  int rc = tlb_stress_xy(h, h->fld[0]);
+  if (rc != TLB_OK) return rc;
+  TLB_ENTER(h);
+  h->launches += launch_x_average(h->d, h->fld[0], Pxy_av, h->st);
+  return check(h);
+}
+
+int tlb_x_average_stress_host(tlb_handle* h, double* Pxy_av) {
+  if (!h || !Pxy_av) return TLB_EINVAL;
+  int rc = tlb_x_average_stress(h, h->fld[1]);
+  if (rc != TLB_OK) return rc;
+  TLB_ENTER(h);
+  cu(h, cudaMemcpyAsync(Pxy_av, h->fld[1], (size_t)h->d.ny * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  return check(h);
+}
+
+// Droplet analysis, first stage (section 2.4): scratch planes fld[1..3] hold the labels, the root lists and the sums.
+int tlb_droplets(tlb_handle* h, double B_th, int32_t* labels, int32_t max_droplets, int32_t* n_droplets, double* stats) {
+  if (!h || !n_droplets || max_droplets < 0 || (max_droplets > 0 && !stats)) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;  // a global analysis: gather the density field of the slabs first
+  const size_t n = (size_t)h->d.nx * h->d.ny;
+  if ((size_t)max_droplets * 4 > n) return TLB_EINVAL;  // root lists and sums live in scratch planes
+  if (!h->has_state) return TLB_ESTATE;
+  TLB_ENTER(h);
+  FusedOut o{};
+  o.rhoA = h->fld[0];
+  int rc = fused_mode(h, 1, o);
+  if (rc != TLB_OK) return rc;
+  int* lab = labels ? labels : reinterpret_cast<int*>(h->fld[1]);
+  h->launches += launch_label_init(h->d, h->fld[0], B_th, lab, h->st);
+  h->launches += launch_label_merge(h->d, lab, h->st);
+  h->launches += launch_label_flatten(h->d, lab, h->st);
+  int* roots = reinterpret_cast<int*>(h->fld[2]);
+  cu(h, cudaMemsetAsync(n_droplets, 0, sizeof(int), h->st));
+  if (max_droplets > 0) cu(h, cudaMemsetAsync(h->fld[3], 0, 3 * sizeof(unsigned long long) * (size_t)max_droplets, h->st));
+  h->launches += launch_droplet_stats(h->d, lab, roots, roots + max_droplets, reinterpret_cast<unsigned long long*>(h->fld[3]),
+                                      max_droplets, n_droplets, stats, h->st);
+  return check(h);
+}
+
+int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_droplets, int32_t* n_droplets, double* stats) {
+  if (!h || !n_droplets || max_droplets < 0 || (max_droplets > 0 && !stats)) return TLB_EINVAL;
+  const size_t n = (size_t)h->d.nx * h->d.ny;
+  if ((size_t)max_droplets * 4 > n) return TLB_EINVAL;  // device copy of the statistics lives in a scratch plane
+  int* lab = reinterpret_cast<int*>(h->fld[1]);
+  double* dstats = h->fld[4];
+  int rc = tlb_droplets(h, B_th, lab, max_droplets, h->n_drop, dstats);
+  if (rc != TLB_OK) return rc;
+  TLB_ENTER(h);
+  if (labels) cu(h, cudaMemcpyAsync(labels, lab, n * sizeof(int), cudaMemcpyDeviceToHost, h->st));
+  cu(h, cudaMemcpyAsync(n_droplets, h->n_drop, sizeof(int), cudaMemcpyDeviceToHost, h->st));
+  if (max_droplets > 0) cu(h, cudaMemcpyAsync(stats, dstats, 4 * sizeof(double) * (size_t)max_droplets, cudaMemcpyDeviceToHost, h->st));
   cu(h, cudaStreamSynchronize(h->st));
   return check(h);
 }
@@ -515,8 +820,8 @@ int64_t tlb_launch_count(const tlb_handle* h) { return h ? h->launches : 0; }
 const char* tlb_error_string(int code) {
   switch (code) {
     case TLB_OK: return "ok";
-    case TLB_EINVAL: return "invalid argument (size, parameter, NULL pointer or workspace too small)";
-    case TLB_ESTATE: return "no state: call tlb_init, tlb_set_fields or tlb_set_populations first";
+    case TLB_EINVAL: return "invalid argument (size, parameter, NULL pointer, workspace too small, or a call this kind of handle does not take)";
+    case TLB_ESTATE: return "no state (call tlb_init, tlb_set_fields or tlb_set_populations first) or slab step calls out of order";
     case TLB_ECUDA: return "CUDA error (see tlb_last_cuda_error); there is no CPU fallback";
     case TLB_EPLACEMENT: return "tlb_init could not place n_droplets by random sequential addition";
   }

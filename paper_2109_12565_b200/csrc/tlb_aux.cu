@@ -119,21 +119,24 @@ __device__ __forceinline__ double uniform01(uint64_t seed, uint64_t stream, uint
   return __dmul_rn((double)(z >> 11), 1.0 / 9007199254740992.0);
 }
 
-// one CTA per droplet: mark the sites of its disc in `inside`
+// one CTA per droplet (centres in coordinates of the whole lattice): mark the sites of its disc in `inside`
 __global__ void raster_kernel(const Dev d, const double* __restrict__ centres, double radius, uint8_t* __restrict__ inside) {
   const double cxd = centres[2 * blockIdx.x], cyd = centres[2 * blockIdx.x + 1];
   const int rr = (int)ceil(radius) + 1;
   const int bx = (int)floor(cxd) - rr, by = (int)floor(cyd) - rr, side = 2 * rr + 2;
   const double r2 = __dmul_rn(radius, radius);
   for (int t = threadIdx.x; t < side * side; t += blockDim.x) {
-    const int y = by + t / side;
-    if (y < 0 || y >= d.ny) continue;
+    const int y = by + t / side;  // row of the whole lattice (droplets never wrap in y)
+    if (y < 0 || y >= d.ny_glob) continue;
     int x = (bx + t % side) % d.nx;
     if (x < 0) x += d.nx;
     double dx = fabs(__dsub_rn((double)x, cxd));
     dx = fmin(dx, __dsub_rn((double)d.nx, dx));
     const double dy = __dsub_rn((double)y, cyd);
-    if (__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)) <= r2) inside[(size_t)y * d.nx + x] = 1;
+    if (__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)) > r2) continue;
+    // local images of that row: one, or none; a slab of a y-periodic lattice may hold it in a wrapped halo row
+    for (int yl = y - d.y_off - (d.per_glob ? d.ny_glob : 0); yl < d.ny; yl += d.ny_glob)
+      if (yl >= 0) inside[(size_t)yl * d.nx + x] = 1;
   }
 }
 
@@ -142,70 +145,41 @@ __global__ void init_fields_kernel(const Dev d, const tlb_params p, uint64_t see
                                    double* __restrict__ T) {
   const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (q >= (size_t)d.nx * d.ny) return;
-  const int x = (int)(q % d.nx), y = (int)(q / d.nx);
+  const int x = (int)(q % d.nx), y = d.gy((int)(q / d.nx));  // the recipe is stated on the whole lattice
+  const uint64_t qg = (uint64_t)y * d.nx + x;
   bool sol = false;  // structured posts, reading R19
   if (p.post_w > 0 && p.post_h > 0 && p.post_period > 0)
-    sol = (x % p.post_period) < p.post_w && (y < p.post_h || y >= d.ny - p.post_h);
+    sol = (x % p.post_period) < p.post_w && (y < p.post_h || y >= d.ny_glob - p.post_h);
   solid[q] = sol ? 1 : 0;
   const bool in = inside[q] != 0;
   double a = in ? p.rho_in : p.rho_out, b = in ? p.rho_out : p.rho_in;
   if (!sol) {
-    a = __dadd_rn(a, __dmul_rn(p.noise_amp, uniform01(seed, 1, q)));
-    b = __dadd_rn(b, __dmul_rn(p.noise_amp, uniform01(seed, 2, q)));
+    a = __dadd_rn(a, __dmul_rn(p.noise_amp, uniform01(seed, 1, qg)));
+    b = __dadd_rn(b, __dmul_rn(p.noise_amp, uniform01(seed, 2, qg)));
   }
   rhoA[q] = a;
   rhoB[q] = b;
   const double yy = __dadd_rn((double)y, 0.5);  // linear profile between the walls, L314
-  T[q] = __dadd_rn(__ddiv_rn(__dmul_rn(__dsub_rn(p.T_top, p.T_bottom), yy), (double)d.ny), p.T_bottom);
+  T[q] = __dadd_rn(__ddiv_rn(__dmul_rn(__dsub_rn(p.T_top, p.T_bottom), yy), (double)d.ny_glob), p.T_bottom);
 }
 
-// ---- observables (a10): mass_A, mass_B, sum |u|^2, sum u_y T, sum d_y T, fluid count ----
-constexpr int kObsThreads = 256;
+// ---- observables (a10): the fused kernel (MODE 3) leaves per-CTA partial sums
+// {mass_A, mass_B, sum |u^(H)|^2, sum u_y^(H) T, sum d_y T, fluid sites}; here they are combined in a fixed order ----
 constexpr int kObsVals = 6;
 
-__device__ __forceinline__ double T_wall(const Dev& d, int y) { return (2 * y < d.ny) ? d.T_bottom : d.T_top; }
-
-__global__ void __launch_bounds__(kObsThreads)
-observables_partial_kernel(const Dev d, const double* __restrict__ rhoA, const double* __restrict__ rhoB,
-                           const double* __restrict__ ux, const double* __restrict__ uy, const double* __restrict__ T,
-                           double* __restrict__ partials) {
-  const int nx = d.nx, ny = d.ny;
-  const size_t n = (size_t)nx * ny;
-  double acc[kObsVals] = {0, 0, 0, 0, 0, 0};
-  for (size_t q = (size_t)blockIdx.x * kObsThreads + threadIdx.x; q < n; q += (size_t)gridDim.x * kObsThreads) {
-    if (d.solid[q]) continue;
-    const int x = (int)(q % nx), y = (int)(q / nx);
-    const double t = T[q];
-    acc[0] += rhoA[q];
-    acc[1] += rhoB[q];
-    acc[2] += ux[q] * ux[q] + uy[q] * uy[q];
-    acc[3] += uy[q] * t;
-    // R10: d_y T = Tface(y + 1/2) - Tface(y - 1/2); Tface = wall temperature at a solid neighbour
-    int yu = y + 1, yd = y - 1;
-    if (d.periodic_y) { yu = wrapi(yu, ny); yd = wrapi(yd, ny); }
-    const double up = fluid_at(d, x, yu) ? 0.5 * (t + T[(size_t)yu * nx + x]) : T_wall(d, yu);
-    const double dn = fluid_at(d, x, yd) ? 0.5 * (t + T[(size_t)yd * nx + x]) : T_wall(d, yd);
-    acc[4] += up - dn;
-    acc[5] += 1.0;
-  }
-  __shared__ double sh[kObsThreads / 32][kObsVals];
-#pragma unroll
-  for (int v = 0; v < kObsVals; v++) {
-    double a = acc[v];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) a += __shfl_down_sync(0xffffffffu, a, o);
-    if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5][v] = a;
-  }
-  __syncthreads();
-  if (threadIdx.x < kObsVals) {
-    double a = 0.0;
-    for (int w = 0; w < kObsThreads / 32; w++) a += sh[w][threadIdx.x];  // fixed order
-    partials[(size_t)blockIdx.x * kObsVals + threadIdx.x] = a;
-  }
+// out4 = {mass_A, mass_B, E, Nu} from the six sums (whole lattice: after an all-reduce over slabs)
+__device__ __forceinline__ void finish_observables(const Dev& d, const double* tot, double* out4) {
+  const double nf = tot[5];
+  const double kappa = (1.0 / d.omega_g - 0.5) / 3.0;  // Eq. (20)
+  const double DT = d.T_bottom - d.T_top;
+  out4[0] = tot[0];
+  out4[1] = tot[1];
+  out4[2] = nf > 0 ? tot[2] / nf : 0.0;                                                                      // L248, R11
+  out4[3] = (nf > 0 && DT != 0.0) ? (tot[3] / nf - kappa * (tot[4] / nf)) / (kappa * DT / d.ny_glob) : 0.0;  // Eq. (24)
 }
 
 __global__ void observables_final_kernel(const Dev d, const double* __restrict__ partials, int n_blocks,
-                                         double* __restrict__ out4) {
+                                         double* __restrict__ sums6, double* __restrict__ out4) {
   __shared__ double tot[kObsVals];
   const int v = threadIdx.x >> 5, lane = threadIdx.x & 31;  // one warp per value, fixed lane order
   double a = 0.0;
@@ -214,21 +188,24 @@ __global__ void observables_final_kernel(const Dev d, const double* __restrict__
   for (int o = 16; o > 0; o >>= 1) a += __shfl_down_sync(0xffffffffu, a, o);
   if (lane == 0) tot[v] = a;
   __syncthreads();
-  if (threadIdx.x == 0) {
-    const double nf = tot[5];
-    const double kappa = (1.0 / d.omega_g - 0.5) / 3.0;  // Eq. (20)
-    const double DT = d.T_bottom - d.T_top;
-    out4[0] = tot[0];
-    out4[1] = tot[1];
-    out4[2] = nf > 0 ? tot[2] / nf : 0.0;
-    out4[3] = (nf > 0 && DT != 0.0) ? (tot[3] / nf - kappa * (tot[4] / nf)) / (kappa * DT / d.ny) : 0.0;  // Eq. (24)
-  }
+  if (threadIdx.x < kObsVals && sums6) sums6[threadIdx.x] = tot[threadIdx.x];
+  if (threadIdx.x == 0 && out4) finish_observables(d, tot, out4);
 }
 
-// one CTA per row: x-average of u_x over the fluid sites (u_av of PAPER L248-250), fixed-order sums
+__global__ void observables_from_sums_kernel(const Dev d, const double* __restrict__ sums6, double* __restrict__ out4) {
+  double tot[kObsVals];
+  for (int v = 0; v < kObsVals; v++) tot[v] = sums6[v];
+  finish_observables(d, tot, out4);
+}
+
+// one CTA per row: x-average of a field plane over the fluid sites (u_av, Pxy_av of PAPER L248-250), fixed-order sums
 __global__ void __launch_bounds__(256)
 x_average_kernel(const Dev d, const double* __restrict__ ux, double* __restrict__ u_av) {
   const int y = blockIdx.x;
+  if (y < d.own0 || y >= d.own1) {  // a slab's halo rows carry no fields
+    if (threadIdx.x == 0) u_av[y] = 0.0;
+    return;
+  }
   double a = 0.0, n = 0.0;
   for (int x = threadIdx.x; x < d.nx; x += 256)
     if (!d.solid[(size_t)y * d.nx + x]) { a += ux[(size_t)y * d.nx + x]; n += 1.0; }
@@ -242,6 +219,168 @@ x_average_kernel(const Dev d, const double* __restrict__ ux, double* __restrict_
     for (int w = 0; w < 8; w++) { ta += sa[w]; tn += sn[w]; }
     u_av[y] = tn > 0.0 ? ta / tn : 0.0;
   }
+}
+
+// ---- y-slab halo rows (tlb.h "Y-SLABS"): the kHalo owned rows next to a face <-> a contiguous buffer
+// [27][kHalo][px] (whole padded rows, ghost columns included).  face 0 = low y, 1 = high y.
+// pack reads the owned rows next to the face; unpack writes the halo rows beyond it.
+template <bool UNPACK, typename ST>
+__global__ void halo_copy_kernel(const Dev d, ST* __restrict__ S, int face, ST* __restrict__ buf) {
+  const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= 27ll * kHalo * d.px) return;
+  const int c = (int)(k % d.px), r = (int)((k / d.px) % kHalo), p = (int)(k / ((long long)d.px * kHalo));
+  int y;
+  if (UNPACK) y = face == 0 ? d.own0 - kHalo + r : d.own1 + r;
+  else y = face == 0 ? d.own0 + r : d.own1 - kHalo + r;
+  const long long o = p * d.plane + (long long)(y + 1) * d.row + c;
+  if (UNPACK) S[o] = buf[k];
+  else buf[k] = S[o];
+}
+
+// ---- droplet analysis, first stage (PAPER section 2.4, reading R22): bulk sites rho_A > B_th, clusters of
+// nearest-neighbour (4-connected) bulk sites, x periodic (y too when the lattice is), label = smallest site index
+// y nx + x of the cluster.  Lock-free union-find: every union hangs the larger root under the smaller one with
+// atomicMin, so parents only decrease and the root of a finished cluster is its smallest index.
+__global__ void label_init_kernel(const Dev d, const double* __restrict__ rhoA, double threshold, int* __restrict__ labels) {
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (size_t)d.nx * d.ny) return;
+  labels[q] = (!d.solid[q] && rhoA[q] > threshold) ? (int)q : -1;
+}
+
+__device__ __forceinline__ int find_root(volatile int* L, int i) {
+  int cur = L[i];
+  if (cur != i) {
+    int prev = i, next;
+    while (cur > (next = L[cur])) {  // path halving; a racing write can only store a smaller ancestor
+      L[prev] = next;
+      prev = cur;
+      cur = next;
+    }
+  }
+  return cur;
+}
+
+__device__ __forceinline__ void unite(int* L, int a, int b) {
+  bool done;
+  do {
+    a = find_root(L, a);
+    b = find_root(L, b);
+    if (a < b) {
+      const int old = atomicMin(&L[b], a);
+      done = old == b;
+      b = old;
+    } else if (b < a) {
+      const int old = atomicMin(&L[a], b);
+      done = old == a;
+      a = old;
+    } else {
+      done = true;
+    }
+  } while (!done);
+}
+
+__global__ void label_merge_kernel(const Dev d, int* __restrict__ labels) {
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (size_t)d.nx * d.ny) return;
+  if (labels[q] < 0) return;
+  const int x = (int)(q % d.nx), y = (int)(q / d.nx);
+  const int xr = x + 1 < d.nx ? x + 1 : 0;
+  if (xr != x) {  // bond to the right-hand neighbour (periodic in x, L147)
+    const int n = y * d.nx + xr;
+    if (labels[n] >= 0) unite(labels, (int)q, n);
+  }
+  int yu = y + 1;
+  if (yu >= d.ny) yu = d.periodic_y ? 0 : -1;
+  if (yu >= 0 && yu != y) {  // bond to the neighbour above
+    const int n = yu * d.nx + x;
+    if (labels[n] >= 0) unite(labels, (int)q, n);
+  }
+}
+
+// Every site takes the root of its tree.  Read-only chase (no path halving here: a halving store of a stale
+// ancestor could land after, and undo, another thread's final write); concurrent final writes only ever replace a
+// parent by the root of the same tree, so every chain stays valid while it is being read.
+__global__ void label_flatten_kernel(const Dev d, int* __restrict__ labels) {
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (size_t)d.nx * d.ny) return;
+  volatile int* L = labels;
+  int cur = L[q];
+  if (cur < 0) return;
+  for (int next = L[cur]; next != cur; next = L[cur]) cur = next;
+  L[q] = cur;
+}
+
+// roots (label == own index) appended in arrival order, then ranked: sorted[rank] = root
+__global__ void droplet_roots_kernel(const Dev d, const int* __restrict__ labels, int* __restrict__ roots, int max_droplets,
+                                     int* __restrict__ n_out) {
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (size_t)d.nx * d.ny) return;
+  if (labels[q] != (int)q) return;
+  const int k = atomicAdd(n_out, 1);
+  if (k < max_droplets) roots[k] = (int)q;
+}
+
+__global__ void droplet_rank_kernel(const int* __restrict__ roots, int max_droplets, const int* __restrict__ n_out,
+                                    int* __restrict__ sorted) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n = min(*n_out, max_droplets);
+  if (i >= n) return;
+  const int r = roots[i];
+  int rank = 0;
+  for (int j = 0; j < n; j++) rank += roots[j] < r;
+  sorted[rank] = r;
+}
+
+// signed minimum-image offset of a from b on a ring of n sites, in [-n/2, n/2)
+__device__ __forceinline__ int min_image(int a, int b, int n) {
+  int dlt = a - b;
+  if (2 * dlt >= n) dlt -= n;
+  else if (2 * dlt < -n) dlt += n;
+  return dlt;
+}
+
+// per droplet: sites, sum of x offsets and of y offsets from the root site -- integer atomics, order-independent
+__global__ void droplet_sums_kernel(const Dev d, const int* __restrict__ labels, const int* __restrict__ sorted,
+                                    int max_droplets, const int* __restrict__ n_out, unsigned long long* __restrict__ sums) {
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (size_t)d.nx * d.ny) return;
+  const int root = labels[q];
+  if (root < 0) return;
+  const int n = min(*n_out, max_droplets);
+  int lo = 0, hi = n;  // lower bound of root in sorted[0, n)
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (sorted[mid] < root) lo = mid + 1;
+    else hi = mid;
+  }
+  if (lo >= n || sorted[lo] != root) return;  // a droplet beyond max_droplets
+  const int x = (int)(q % d.nx), y = (int)(q / d.nx), xr = root % d.nx, yr = root / d.nx;
+  const long long dx = min_image(x, xr, d.nx);
+  const long long dy = d.periodic_y ? min_image(y, yr, d.ny) : y - yr;
+  atomicAdd(&sums[3 * lo + 0], 1ull);
+  atomicAdd(&sums[3 * lo + 1], (unsigned long long)dx);  // two's complement: wraps to the signed sum
+  atomicAdd(&sums[3 * lo + 2], (unsigned long long)dy);
+}
+
+// stats[k] = {label, sites, centre x, centre y} in ascending label order; centre = root + mean offset, wrapped
+__global__ void droplet_finish_kernel(const Dev d, const int* __restrict__ sorted, const unsigned long long* __restrict__ sums,
+                                      int max_droplets, const int* __restrict__ n_out, double* __restrict__ stats) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= min(*n_out, max_droplets)) return;
+  const int root = sorted[k];
+  const double cnt = (double)(long long)sums[3 * k];
+  double cxm = (double)(root % d.nx) + __ddiv_rn((double)(long long)sums[3 * k + 1], cnt);
+  double cym = (double)(root / d.nx) + __ddiv_rn((double)(long long)sums[3 * k + 2], cnt);
+  if (cxm < 0.0) cxm += (double)d.nx;
+  if (cxm >= (double)d.nx) cxm -= (double)d.nx;
+  if (d.periodic_y) {
+    if (cym < 0.0) cym += (double)d.ny;
+    if (cym >= (double)d.ny) cym -= (double)d.ny;
+  }
+  stats[4 * k + 0] = (double)root;
+  stats[4 * k + 1] = cnt;
+  stats[4 * k + 2] = cxm;
+  stats[4 * k + 3] = cym;
 }
 
 inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
@@ -273,15 +412,13 @@ int launch_copy_g(const Dev& d, const void* Ssrc, void* Sdst, cudaStream_t st) {
   return 1;
 }
 int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st) {
-  cudaMemsetAsync(count, 0, sizeof(int), st);
   build_links_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, sites, count);
   pad_mask_kernel<<<blocks_for((long long)d.px * d.ny, 256), 256, 0, st>>>(d, solidp);
   return 2;
 }
 int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* centres, int n_centres, uint8_t* inside,
                 uint8_t* solid, double* rhoA, double* rhoB, double* T, cudaStream_t st) {
-  int launches = 1;
-  cudaMemsetAsync(inside, 0, (size_t)d.nx * d.ny, st);
+  int launches = 1;  // `inside` was zeroed by the caller
   if (n_centres > 0) {
     raster_kernel<<<n_centres, 128, 0, st>>>(d, centres, p.droplet_radius, inside);
     launches++;
@@ -289,15 +426,53 @@ int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* 
   init_fields_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, p, seed, inside, solid, rhoA, rhoB, T);
   return launches;
 }
-int launch_x_average(const Dev& d, const double* ux, double* u_av, cudaStream_t st) {
-  x_average_kernel<<<d.ny, 256, 0, st>>>(d, ux, u_av);
+int launch_x_average(const Dev& d, const double* plane, double* av, cudaStream_t st) {
+  x_average_kernel<<<d.ny, 256, 0, st>>>(d, plane, av);
   return 1;
 }
-int launch_observables(const Dev& d, const double* rhoA, const double* rhoB, const double* ux, const double* uy,
-                       const double* T, double* partials, int n_blocks, double* out4, cudaStream_t st) {
-  observables_partial_kernel<<<n_blocks, kObsThreads, 0, st>>>(d, rhoA, rhoB, ux, uy, T, partials);
-  observables_final_kernel<<<1, 32 * kObsVals, 0, st>>>(d, partials, n_blocks, out4);
-  return 2;
+int launch_observables_final(const Dev& d, const double* partials, int n_blocks, double* sums6, double* out4,
+                             cudaStream_t st) {
+  observables_final_kernel<<<1, 32 * kObsVals, 0, st>>>(d, partials, n_blocks, sums6, out4);
+  return 1;
+}
+int launch_observables_from_sums(const Dev& d, const double* sums6, double* out4, cudaStream_t st) {
+  observables_from_sums_kernel<<<1, 1, 0, st>>>(d, sums6, out4);
+  return 1;
+}
+int launch_halo_pack(const Dev& d, const void* S, int face, void* buf, cudaStream_t st) {
+  const long long n = 27ll * kHalo * d.px;
+  if (d.prec == 32) halo_copy_kernel<false, float><<<blocks_for(n, 256), 256, 0, st>>>(d, const_cast<float*>(static_cast<const float*>(S)), face, static_cast<float*>(buf));
+  else halo_copy_kernel<false, double><<<blocks_for(n, 256), 256, 0, st>>>(d, const_cast<double*>(static_cast<const double*>(S)), face, static_cast<double*>(buf));
+  return 1;
+}
+int launch_halo_unpack(const Dev& d, void* S, int face, const void* buf, cudaStream_t st) {
+  const long long n = 27ll * kHalo * d.px;
+  if (d.prec == 32) halo_copy_kernel<true, float><<<blocks_for(n, 256), 256, 0, st>>>(d, static_cast<float*>(S), face, const_cast<float*>(static_cast<const float*>(buf)));
+  else halo_copy_kernel<true, double><<<blocks_for(n, 256), 256, 0, st>>>(d, static_cast<double*>(S), face, const_cast<double*>(static_cast<const double*>(buf)));
+  return 1;
+}
+int launch_label_init(const Dev& d, const double* rhoA, double threshold, int* labels, cudaStream_t st) {
+  label_init_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, rhoA, threshold, labels);
+  return 1;
+}
+int launch_label_merge(const Dev& d, int* labels, cudaStream_t st) {
+  label_merge_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, labels);
+  return 1;
+}
+int launch_label_flatten(const Dev& d, int* labels, cudaStream_t st) {
+  label_flatten_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, labels);
+  return 1;
+}
+// roots / sorted: [max_droplets] ints each, sums: [max_droplets][3] 64-bit (zeroed by the caller, like n_out);
+// n_out: the number of droplets found; if it exceeds max_droplets the statistics are not meaningful
+int launch_droplet_stats(const Dev& d, const int* labels, int* roots, int* sorted, unsigned long long* sums,
+                         int max_droplets, int* n_out, double* stats, cudaStream_t st) {
+  const unsigned nb = blocks_for((long long)d.nx * d.ny, 256);
+  droplet_roots_kernel<<<nb, 256, 0, st>>>(d, labels, roots, max_droplets, n_out);
+  droplet_rank_kernel<<<blocks_for(max_droplets, 256), 256, 0, st>>>(roots, max_droplets, n_out, sorted);
+  droplet_sums_kernel<<<nb, 256, 0, st>>>(d, labels, sorted, max_droplets, n_out, sums);
+  droplet_finish_kernel<<<blocks_for(max_droplets, 256), 256, 0, st>>>(d, sorted, sums, max_droplets, n_out, stats);
+  return 4;
 }
 
 }  // namespace tlb

@@ -31,20 +31,22 @@ __host__ __device__ constexpr int opp(int i) { return i == 0 ? 0 : (i <= 4 ? ((i
 __host__ __device__ constexpr double wq(int i) { return i == 0 ? 4.0 / 9.0 : (i <= 4 ? 1.0 / 9.0 : 1.0 / 36.0); }
 
 // fused-kernel geometry (see tlb_step.cu)
-#ifndef TLB_KW
-#define TLB_KW 128
-#endif
-constexpr int kW = TLB_KW;              // strip width = lattice columns per CTA (two threads per column)
+constexpr int kW = 128;                 // strip width = lattice columns per CTA (two threads per column)
 constexpr int kHX = 4;                  // columns fetched beyond the strip on each side (3 needed; 4 keeps 16-byte alignment)
 constexpr int kCopyW = kW + 2 * kHX;    // doubles per plane-row copy
 constexpr int kSlots = 4;               // rows of the 18 fluid planes resident in shared memory
 constexpr int kRingRows = 6;            // rows of rho / psi kept in shared memory
 constexpr int kXL = 16;                 // padded-row offset of lattice column 0
 constexpr int kGhost = kHX;             // ghost columns kept valid on each side
+constexpr int kHalo = 3;                // halo rows per interior face of a y-slab (see tlb.h, "Y-SLABS")
 
 // Everything a kernel needs, passed by value (lives in the constant bank of the launch).
 struct Dev {
-  int nx, ny;
+  int nx, ny;            // local lattice; for a y-slab ny counts the halo rows too
+  int y_off, ny_glob;    // y-slab: global row of local row 0 and rows of the whole lattice (else 0, ny)
+  int per_glob;          // the whole lattice is periodic in y (a slab of it is not: its faces import halo rows)
+  int wall_lo, wall_hi;  // is there a flat wall beyond local row 0 / ny - 1 (else: periodic wrap, or a slab face)
+  int own0, own1;        // local rows this handle computes (a slab imports the others from its neighbours)
   int px;                // padded row pitch in doubles (and in bytes of the padded mask)
   int periodic_y, thermal;
   int prec;              // storage precision of the populations: 64 (double) or 32 (float; arithmetic stays fp64)
@@ -60,6 +62,13 @@ struct Dev {
   const uint8_t* solid;  // [ny][nx]   flag field in the API layout (L286)
   const uint8_t* solidp; // [ny][px]   the same with ghost columns, lattice column x at kXL + x
 
+  // wall temperature carried by a solid node of local row y (R8): lower half of the whole lattice -> T_bottom
+  __host__ __device__ int gy(int y) const {  // row of the whole lattice that local row y is
+    int g = y + y_off;
+    if (per_glob) { g %= ny_glob; if (g < 0) g += ny_glob; }
+    return g;
+  }
+  __host__ __device__ double T_wall(int y) const { return (2 * gy(y) < ny_glob) ? T_bottom : T_top; }
   // offset of lattice node (x, y) inside a plane; x in [-kXL, px - kXL), y in [-1, ny]
   __host__ __device__ long long at(int x, int y) const { return (long long)(y + 1) * row + kXL + x; }
 };
@@ -69,10 +78,17 @@ __host__ __device__ inline int padded_pitch(int nx) {
   return kXL + strips * kW + 16;  // multiple of 16; room for the last strip's copy overhang
 }
 
+// outputs of the fused kernel's non-stepping modes (any pointer may be null)
+struct FusedOut {
+  double *rhoA, *rhoB, *ux, *uy, *T;  // MODE 1: [ny][nx] planes
+  double* pxy;                        // MODE 2
+  double* partials;                   // MODE 3: [CTAs][6] {mass_A, mass_B, sum |u|^2, sum u_y T, sum d_y T, fluid sites}
+};
+
 // launchers (each returns the number of kernels it launched)
-int launch_step(const Dev& d, const void* Sin, void* Sout, int seg_rows, cudaStream_t st);
-int launch_fields(const Dev& d, const void* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
-                  cudaStream_t st);
+int launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
+                 cudaStream_t st);
+int fused_grid_ctas(const Dev& d, int seg_rows, int rows);  // CTAs launch_fused uses for `rows` rows
 int launch_boundary(const Dev& d, void* S, const int* sites, int n_sites, cudaStream_t st);
 int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st);
 int launch_scatter(const Dev& d, const double* fA, const double* fB, const double* g, void* S, cudaStream_t st);
@@ -82,11 +98,17 @@ int launch_set_fields(const Dev& d, const double* rhoA, const double* rhoB, cons
 int launch_copy_g(const Dev& d, const void* Ssrc, void* Sdst, cudaStream_t st);
 int launch_init(const Dev& d, const tlb_params& p, uint64_t seed, const double* centres, int n_centres,
                 uint8_t* inside_scratch, uint8_t* solid, double* rhoA, double* rhoB, double* T, cudaStream_t st);
-int launch_observables(const Dev& d, const double* rhoA, const double* rhoB, const double* ux, const double* uy,
-                       const double* T, double* partials, int n_blocks, double* out4, cudaStream_t st);
-int launch_x_average(const Dev& d, const double* ux, double* u_av, cudaStream_t st);
+int launch_observables_final(const Dev& d, const double* partials, int n_blocks, double* sums6, double* out4, cudaStream_t st);
+int launch_observables_from_sums(const Dev& d, const double* sums6, double* out4, cudaStream_t st);
+int launch_x_average(const Dev& d, const double* plane, double* av, cudaStream_t st);
+int launch_halo_pack(const Dev& d, const void* S, int face, void* buf, cudaStream_t st);
+int launch_halo_unpack(const Dev& d, void* S, int face, const void* buf, cudaStream_t st);
+int launch_label_init(const Dev& d, const double* rhoA, double threshold, int* labels, cudaStream_t st);
+int launch_label_merge(const Dev& d, int* labels, cudaStream_t st);
+int launch_label_flatten(const Dev& d, int* labels, cudaStream_t st);
+int launch_droplet_stats(const Dev& d, const int* labels, int* roots, int* sorted, unsigned long long* sums,
+                         int max_droplets, int* n_out, double* stats, cudaStream_t st);
 int configure_kernels();  // opt in to the dynamic shared memory the fused kernel needs; 0 on success
 int default_seg_rows(int nx, int ny);
-constexpr int kObsBlocks = 592; // 4 per SM on 148 SMs
 
 }  // namespace tlb

@@ -1,8 +1,8 @@
 // tlb_step.cu -- the fused force + collide + stream kernel (PAPER Eqs. (1)-(22)) and the
 // wall / obstacle boundary kernel (L151, L155, L314), hand-written for sm_100a.
 //
-// Fused kernel, "strip marching with an asynchronous row pipeline".  A CTA of kW threads owns kW
-// lattice columns and marches over a segment of rows.  For every row r one elected thread issues
+// Fused kernel, "strip marching with an asynchronous row pipeline".  A CTA of 2 kW threads (two per
+// lattice column, one per species) owns kW columns and marches over a segment of rows.  For every row r one elected thread issues
 // 18 bulk asynchronous copies (cp.async.bulk, the 1-D TMA path; SASS UBLKCP) that bring the strip
 // of the 18 fluid planes, already shifted in y by the pull rule f_i(x, r) = S_i(x - c_i), into a
 // 4-slot ring in shared memory and complete on an mbarrier; the x shift is applied when threads
@@ -15,12 +15,10 @@
 //       populations at (x, y).
 // Streaming (Eq. (1)) is the gather of the next step, so stores are never shifted.  The 9 thermal
 // planes are only needed in (2) and go straight to registers (LDG issued before the row barrier).
-// The four warps of a CTA never meet at a CTA-wide barrier: each warp keeps its own rho / psi ring
-// for its 32 columns plus a 2-cell halo (the 4 halo columns are recomputed, not exchanged), waits
+// The eight warps of a CTA never meet at a CTA-wide barrier: each warp keeps its own rho / psi ring
+// for its 16 columns plus a 2-cell halo (the 4 halo columns are recomputed, not exchanged), waits
 // on the mbarrier of the row it needs, and counts itself out of the slot it has finished with; the
 // last warp out issues the copy of row r+2 into that slot, a full row of compute ahead of its use.
-#include <cstdlib>
-
 #include "tlb_internal.cuh"
 
 namespace tlb {
@@ -67,11 +65,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
           smem_u32(dst)),
       "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
-}
-// L2 prefetch of `bytes` (multiple of 16, 16-byte aligned): starts the HBM read rows ahead of the copy
-// that needs shared memory, so the depth of the read queue is not bounded by the shared-memory ring
-__device__ __forceinline__ void prefetch_l2(const void* src, uint32_t bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ double ldg_stream(const double* a, uint64_t policy) {
   double v;
@@ -129,10 +122,6 @@ __device__ __forceinline__ int wrap_row(int r, int ny) {
   return r < 0 ? r + ny : r;
 }
 
-#ifndef TLB_PREF_D
-#define TLB_PREF_D 0
-#endif
-constexpr int kPrefetchRows = TLB_PREF_D;  // rows an optional HBM -> L2 prefetch runs ahead of the copies (0 = off: measured 3 % faster)
 constexpr int kCtasPerSM = 256 / kW;     // shared memory allows 2 CTAs of 128 columns (or 1 of 256) per SM
 constexpr int kThreads = 2 * kW;       // two threads per lattice column: lane 2k = species A, 2k+1 = species B
 constexpr int kWarps = kThreads / 32;  // 8
@@ -177,16 +166,21 @@ __device__ __forceinline__ double relax_tau1(double owd, double cu, double usq) 
 
 }  // namespace
 
-// MODE 0: time step (writes Sout).  MODE 1: hydrodynamic fields of the current state.
+// MODE 0: time step (writes Sout).  MODE 1: hydrodynamic fields of the current state.  MODE 2: the stress
+// field P_xy (reading R21).  MODE 3: per-CTA partial sums of the observables (a10), reduced in the same pass.
 // Work split inside a lane pair (s = lane & 1): lane s owns species s -- its density and psi^s
 // (phase 1), its force, shifted velocity, collision and 9 stores (phase 2) -- and half of the thermal
 // set: s = 0 takes g_0, g_1, g_2, g_5, g_6, s = 1 the opposite directions g_3, g_4, g_7, g_8, so both
 // lanes run the same code on (c_i, u) and (-c_i, -u).  Partial sums (j, F, T) cross by one shuffle.
 template <int MODE, bool PERIODIC, typename ST>
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
-fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int seg_rows,
-             double* __restrict__ oRA, double* __restrict__ oRB, double* __restrict__ oUx, double* __restrict__ oUy,
-             double* __restrict__ oT) {
+fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int seg_rows, int ya, int yb,
+             const FusedOut out) {
+  double* __restrict__ const oRA = out.rhoA;
+  double* __restrict__ const oRB = out.rhoB;
+  double* __restrict__ const oUx = out.ux;
+  double* __restrict__ const oUy = out.uy;
+  double* __restrict__ const oT = out.T;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   Smem<ST>& sm = *reinterpret_cast<Smem<ST>*>(smem_raw);
   constexpr int kSW = SlotW<ST>::v, kB = (int)sizeof(ST);
@@ -197,8 +191,8 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
   const int x0 = blockIdx.x * kW;
   const int xw = x0 + kWC * wid - 2;          // lattice column of this warp's ring column 0
   const int x = xw + 2 + k;                   // phase-2 column of this lane pair
-  const int y0 = blockIdx.y * seg_rows;
-  const int y1 = min(ny, y0 + seg_rows);
+  const int y0 = ya + blockIdx.y * seg_rows;  // this CTA marches rows [y0, y1) of the launch's range [ya, yb)
+  const int y1 = min(yb, y0 + seg_rows);
   const long long plane = d.plane;
   const long long planeB = plane * kB, rowB = d.row * kB;
   const uint64_t pol = policy_evict_first();  // every line of Sin is dead once read, Sout until the next step
@@ -234,28 +228,8 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
         bulk_g2s(&sm.f[q & 3][l * 9 + i][0], Sin + (l * 9 + i) * plane + o, kCopyW * kB, bar, pol);
       }
   };
-  // elected lane: start the HBM -> L2 read of all 27 source plane rows of target row r
-  auto prefetch = [&](int q) {
-    const int r = y0 - 2 + q;
-    if (!row_valid(r)) return;
-    const int rr = PERIODIC ? wrap_row(r, ny) : r;
-    int rm = rr - 1, rp = rr + 1;
-    if (PERIODIC) {
-      if (rm < 0) rm = ny - 1;
-      if (rp >= ny) rp = 0;
-    }
-    const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
-    const int np = (d.thermal && q >= 2 && q < q_end - 2) ? 27 : 18;  // g only for rows that reach phase 2
-#pragma unroll
-    for (int p = 0; p < 27; p++) {
-      const int i = p % 9;
-      const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-      if (p < np) prefetch_l2(Sin + p * plane + o, kCopyW * kB);
-    }
-  };
   if (t == 0) {
     for (int q = 0; q < 4 && q < q_end; q++) issue(q);
-    for (int q = 4; q < 4 + kPrefetchRows && q < q_end; q++) prefetch(q);
   }
 
   // phase-1 tasks of this lane: ring column k and, for lanes < 8, ring column 16 + k; species s
@@ -288,7 +262,8 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 
   // thermal populations of (x, y).  Lane s = 0 reads
   // g_0, g_1, g_2, g_5, g_6 at x - c_i; lane s = 1 the opposite directions at x + c_i.
-  double g0, ga, gb, gc, gd;
+  double g0 = 0.0, ga = 0.0, gb = 0.0, gc = 0.0, gd = 0.0;
+  double acc0 = 0.0, acc1 = 0.0, acc2 = 0.0;  // MODE 3: s = 0 {mass_A, sum |u^(H)|^2, sum u_y^(H) T}; s = 1 {mass_B, sum d_y T, fluid sites}
   auto load_g = [&](int y) {
     long long rofs = s ? rowB : -rowB;  // row y - c_y of this lane's c_y = +-1 directions
     if (PERIODIC) {
@@ -314,7 +289,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     }
     const int y = r - 2;        // row of phase 2
     const bool do2 = y >= y0;
-    if (do2) load_g(y);  // consumed after the force stencil (issuing it a row earlier measured slower)
+    if (do2 && (MODE == 1 || MODE == 3 || d.thermal)) load_g(y);  // consumed after the force stencil (a row earlier measured slower)
     // ---- (1) rho_s, psi^s_s of row r (Eqs. (4), (12)); wall values at solid / out-of-domain nodes (L155, R9)
     if (valid) {
       mbar_wait(&sm.full[slot], (parity >> slot) & 1u);
@@ -349,7 +324,6 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
     if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1) {  // last warp out: the slot is free
       if (q + 2 < q_end) issue(q + 2);
-      if (q + 2 + kPrefetchRows < q_end) prefetch(q + 2 + kPrefetchRows);
     }
     if (!do2) continue;
 
@@ -414,10 +388,28 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
         } else {  // solid site: report the wall values
           if (o1) o1[o] = rho_wall;
           if (o2) o2[o] = 0.0;
-          if (!s && oT) oT[o] = (2 * y < ny) ? d.T_bottom : d.T_top;
+          if (!s && oT) oT[o] = d.T_wall(y);
+        }
+      }
+    } else if (MODE == 3) {
+      // a10: mass_l (north_star), E (L248, R11), Nu (Eq. (24), R10).  R10's face differences telescope over every
+      // fluid-fluid link, so sum_fluid d_y T = sum over fluid sites of [solid above] T_w(y + 1) - [solid below] T_w(y - 1).
+      if (fluid) {
+        const int rqp = (q + kRingRows - 1) % kRingRows, rqm = (q + kRingRows - 3) % kRingRows;  // ring rows of y + 1, y - 1
+        int yu = y + 1, yd = y - 1;
+        if (PERIODIC) { yu = yu >= ny ? 0 : yu; yd = yd < 0 ? ny - 1 : yd; }
+        acc0 += rl;
+        if (!s) {
+          acc1 += uHx * uHx + uHy * uHy;
+          acc2 += uHy * T;
+        } else {
+          acc1 += (flag[rqp][cc] ? d.T_wall(yu) : 0.0) - (flag[rqm][cc] ? d.T_wall(yd) : 0.0);
+          acc2 += 1.0;
         }
       }
     } else {
+      // kinetic part of P_xy (R21): momentum flux sum_i c_ix c_iy f_i of the populations arriving at (x, y) ...
+      const double kpre = (f[5] - f[6]) + (f[7] - f[8]);
       // own species: Eq. (6) shifted velocity, Eqs. (2), (3)
       {
         const double vx = ux + Fx * invl, vy = uy + Fy * invl;
@@ -445,8 +437,30 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
           f[8] = relax(f[8], w5, vx - vy, usq, om1);
         }
       }
+      if (MODE == 2) {
+        // ... averaged with that of the populations leaving it, plus the interaction part: for every coupling
+        // F = -G psi(x) sum_c k(c) psi'(x + c) c the tensor (G / 2) psi(x) sum_c k(c) psi'(x + c) c_x c_y.  Terms
+        // of c and -c have the same c_x c_y and are paired; only |c|^2 = 2, 5, 8 have c_x c_y != 0.
+        const double kpost = (f[5] - f[6]) + (f[7] - f[8]);
+        double Is = 0.0, Ix = 0.0;
+#pragma unroll
+        for (int dy = 1; dy <= 2; dy++) {
+          const int slp = (q + kRingRows - 2 + dy) % kRingRows, slm = (q + kRingRows - 2 - dy) % kRingRows;
+#pragma unroll
+          for (int dx = -2; dx <= 2; dx++) {
+            if (dx == 0) continue;
+            const int c2 = dx * dx + dy * dy;
+            const double kk = c2 == 2 ? k2 : c2 == 5 ? k5 : k8;
+            Is += (kk * (dx * dy)) * (psi_r[slp][cc + dx][s] + psi_r[slm][cc - dx][s]);
+            if (c2 == 2) Ix += (w_c2(2) * (dx * dy)) * (rho_r[slp][cc + dx][1 - s] + rho_r[slm][cc - dx][1 - s]);
+          }
+        }
+        const double pl_xy = 0.5 * (kpre + kpost) + 0.5 * (pl * Is + gx * rl * Ix);
+        const double pxy = pl_xy + pair(pl_xy);
+        if (!s && x < nx) out.pxy[(size_t)y * nx + x] = fluid ? pxy : 0.0;
+      }
       // own half of the thermal set: Eqs. (16), (18) with u^(H); directions sgn * {c_1, c_2, c_5, c_6}
-      if (d.thermal) {
+      if (MODE == 0 && d.thermal) {
         const double vx = sgn * uHx, vy = sgn * uHy;
         const double usq = 1.0 - 1.5 * (uHx * uHx + uHy * uHy);
         const double w0 = d.omega_g * (wq(0) * T), w1 = d.omega_g * (wq(1) * T), w5 = d.omega_g * (wq(5) * T);
@@ -464,7 +478,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
           gd = relax(gd, w5, -vx + vy, usq, om1g);
         }
       }
-      if (fluid) {
+      if (MODE == 0 && fluid) {
 #pragma unroll
         for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<ST*>(opf + i * planeB), f[i], pol);
         if (d.thermal) {
@@ -495,6 +509,30 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     opf += rowB;
     opg += rowB;
   }
+  if (MODE == 3) {
+    // warp-level reduction over the 16 lanes of each species (fixed butterfly), then the 8 warps in a fixed order
+    __syncthreads();  // all warps are done with the rings; reuse the first ring as scratch
+    double* scratch = &sm.rho[0][0][0][0];
+#pragma unroll
+    for (int o = 2; o < 32; o <<= 1) {
+      acc0 += __shfl_xor_sync(0xffffffffu, acc0, o);
+      acc1 += __shfl_xor_sync(0xffffffffu, acc1, o);
+      acc2 += __shfl_xor_sync(0xffffffffu, acc2, o);
+    }
+    if (lane < 2) {
+      scratch[(wid * 2 + lane) * 3 + 0] = acc0;
+      scratch[(wid * 2 + lane) * 3 + 1] = acc1;
+      scratch[(wid * 2 + lane) * 3 + 2] = acc2;
+    }
+    __syncthreads();
+    if (t < 6) {
+      double a = 0.0;
+      for (int w = 0; w < kWarps; w++) a += scratch[(w * 2 + t / 3) * 3 + t % 3];
+      // order {mass_A, mass_B, sum u^2, sum u_y T, sum d_y T, count}
+      const int slot = t == 0 ? 0 : t == 1 ? 2 : t == 2 ? 3 : t == 3 ? 1 : t;
+      out.partials[((size_t)blockIdx.y * gridDim.x + blockIdx.x) * 6 + slot] = a;
+    }
+  }
 }
 
 // Boundary kernel (a9): fills the ghost rows beyond flat walls and the surface of obstacles with the
@@ -508,14 +546,14 @@ template <typename ST>
 __global__ void __launch_bounds__(256)
 boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, int n_sites) {
   const int nx = d.nx, ny = d.ny;
-  const int n_ghost = d.periodic_y ? 0 : 2 * nx;
+  const int n_lo = d.wall_lo ? nx : 0, n_ghost = n_lo + (d.wall_hi ? nx : 0);  // ghost rows exist beyond flat walls only
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   const int node = k >> 3, i = (k & 7) + 1;
   if (node >= n_ghost + n_sites) return;
   int sx, sy;  // lattice coordinates of the solid node, sy in -1..ny
   if (node < n_ghost) {
-    sx = node < nx ? node : node - nx;
-    sy = node < nx ? -1 : ny;
+    sx = node < n_lo ? node : node - n_lo;
+    sy = node < n_lo ? -1 : ny;
   } else {
     const int s = sites[node - n_ghost];
     sx = s % nx;
@@ -526,7 +564,7 @@ boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, 
   if (d.periodic_y) y = y < 0 ? y + ny : (y >= ny ? y - ny : y);
   if (y < 0 || y >= ny) return;
   if (d.solid[(size_t)y * nx + x]) return;
-  const double Tw = (2 * sy < ny) ? d.T_bottom : d.T_top;
+  const double Tw = d.T_wall(sy);
   const long long plane = d.plane;
   const long long os = d.at(sx, sy), ox = d.at(x, y);
   const int io = opp(i);
@@ -554,17 +592,21 @@ boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, 
   }
 }
 
-static dim3 strip_grid(const Dev& d, int seg_rows) {
-  return dim3((d.nx + kW - 1) / kW, (d.ny + seg_rows - 1) / seg_rows);
+static dim3 strip_grid(const Dev& d, int seg_rows, int rows) {
+  return dim3((d.nx + kW - 1) / kW, (rows + seg_rows - 1) / seg_rows);
 }
 
 template <typename ST>
 static cudaError_t configure_for() {
   const int bytes = (int)sizeof(Smem<ST>);
-  cudaError_t e = cudaFuncSetAttribute(fused_kernel<0, false, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<0, true, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, false, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fused_kernel<1, true, ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  cudaError_t e = cudaSuccess;
+  auto set = [&](auto* k) {
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  };
+  set(fused_kernel<0, false, ST>); set(fused_kernel<0, true, ST>);
+  set(fused_kernel<1, false, ST>); set(fused_kernel<1, true, ST>);
+  set(fused_kernel<2, false, ST>); set(fused_kernel<2, true, ST>);
+  set(fused_kernel<3, false, ST>); set(fused_kernel<3, true, ST>);
   return e;
 }
 
@@ -577,10 +619,7 @@ int configure_kernels() {
 // Rows per CTA segment: strips x segments should fill whole waves of 2 CTAs per SM on 148 SMs with
 // as few segments as possible (each segment re-reads 4 warm-up rows), never below kMinSegRows rows
 // (small lattices are bound by the latency of the serial march, not by the redundant rows).
-#ifndef TLB_MIN_SEG
-#define TLB_MIN_SEG 2
-#endif
-constexpr int kMinSegRows = TLB_MIN_SEG;
+constexpr int kMinSegRows = 2;
 int default_seg_rows(int nx, int ny) {
   const int strips = (nx + kW - 1) / kW, slots = kCtasPerSM * 148;
   int best_seg = ny;
@@ -601,38 +640,40 @@ int default_seg_rows(int nx, int ny) {
   return best_seg;
 }
 
-template <typename ST>
-static void launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, double* rhoA, double* rhoB,
-                         double* ux, double* uy, double* T, cudaStream_t st) {
+int fused_grid_ctas(const Dev& d, int seg_rows, int rows) {
+  const dim3 g = strip_grid(d, seg_rows, rows);
+  return (int)(g.x * g.y);
+}
+
+template <int MODE, typename ST>
+static void launch_mode(const Dev& d, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
+                        cudaStream_t st) {
   const ST* in = static_cast<const ST*>(Sin);
-  ST* out = static_cast<ST*>(Sout);
-  const dim3 g = strip_grid(d, seg_rows);
+  ST* o = static_cast<ST*>(Sout);
+  const dim3 g = strip_grid(d, seg_rows, yb - ya);
   const size_t sm = sizeof(Smem<ST>);
-  if (mode == 0) {
-    if (d.periodic_y) fused_kernel<0, true, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
-    else fused_kernel<0, false, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
-  } else {
-    if (d.periodic_y) fused_kernel<1, true, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
-    else fused_kernel<1, false, ST><<<g, kThreads, sm, st>>>(d, in, out, seg_rows, rhoA, rhoB, ux, uy, T);
+  if (d.periodic_y) fused_kernel<MODE, true, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out);
+  else fused_kernel<MODE, false, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out);
+}
+
+// Launch the fused kernel in `mode` on local rows [ya, yb); returns the number of launches (0 for an empty range).
+int launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
+                 cudaStream_t st) {
+  if (yb <= ya) return 0;
+  if (seg_rows > yb - ya) seg_rows = yb - ya;
+  if (seg_rows < 1) seg_rows = 1;
+  const bool f32 = d.prec == 32;
+  switch (mode) {
+    case 0: f32 ? launch_mode<0, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<0, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
+    case 1: f32 ? launch_mode<1, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<1, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
+    case 2: f32 ? launch_mode<2, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<2, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
+    default: f32 ? launch_mode<3, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<3, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
   }
-}
-
-int launch_step(const Dev& d, const void* Sin, void* Sout, int seg_rows, cudaStream_t st) {
-  if (d.prec == 32) launch_fused<float>(d, 0, Sin, Sout, seg_rows, nullptr, nullptr, nullptr, nullptr, nullptr, st);
-  else launch_fused<double>(d, 0, Sin, Sout, seg_rows, nullptr, nullptr, nullptr, nullptr, nullptr, st);
-  return 1;
-}
-
-int launch_fields(const Dev& d, const void* S, double* rhoA, double* rhoB, double* ux, double* uy, double* T,
-                  cudaStream_t st) {
-  const int seg_rows = default_seg_rows(d.nx, d.ny);
-  if (d.prec == 32) launch_fused<float>(d, 1, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T, st);
-  else launch_fused<double>(d, 1, S, nullptr, seg_rows, rhoA, rhoB, ux, uy, T, st);
   return 1;
 }
 
 int launch_boundary(const Dev& d, void* S, const int* sites, int n_sites, cudaStream_t st) {
-  const long long n = 8ll * ((d.periodic_y ? 0 : 2 * d.nx) + n_sites);
+  const long long n = 8ll * ((d.wall_lo ? d.nx : 0) + (d.wall_hi ? d.nx : 0) + n_sites);
   if (n == 0) return 0;
   const unsigned blocks = (unsigned)((n + 255) / 256);
   if (d.prec == 32) boundary_kernel<float><<<blocks, 256, 0, st>>>(d, static_cast<float*>(S), sites, n_sites);
