@@ -66,6 +66,10 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
+// L2 prefetch of `bytes` (multiple of 16, 16-byte aligned): starts the HBM read rows ahead of the loads that use it
+__device__ __forceinline__ void prefetch_l2(const void* src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ double ldg_stream(const double* a, uint64_t policy) {
   double v;
   asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(policy));
@@ -122,6 +126,12 @@ __device__ __forceinline__ int wrap_row(int r, int ny) {
   return r < 0 ? r + ny : r;
 }
 
+// The thermal populations reach the lanes through plain loads issued in the iteration that uses them, so their
+// latency is exposed unless the lines are already in L2: the warp that re-arms a slot also prefetches the 9 thermal
+// plane rows of the row that reaches phase 2 kGPrefetchRows iterations later (measured on config 4, same box:
+// 0.717 ms without, 0.724 / 0.695 / 0.684 / 0.682 / 0.684 / 0.690 / 0.714 ms at 1 / 2 / 3 / 4 / 6 / 8 / 12 rows;
+// prefetching the 18 fluid plane rows as well costs 5 %: the bulk copies already run a row and a half ahead).
+constexpr int kGPrefetchRows = 4;
 constexpr int kCtasPerSM = 256 / kW;     // shared memory allows 2 CTAs of 128 columns (or 1 of 256) per SM
 constexpr int kThreads = 2 * kW;       // two threads per lattice column: lane 2k = species A, 2k+1 = species B
 constexpr int kWarps = kThreads / 32;  // 8
@@ -324,6 +334,20 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
     if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1) {  // last warp out: the slot is free
       if (q + 2 < q_end) issue(q + 2);
+      const int yp = y0 + q - 4 + kGPrefetchRows;  // phase 2 of row yp runs kGPrefetchRows iterations from now
+      if ((MODE == 1 || MODE == 3 || d.thermal) && yp < y1) {
+        int ym = yp - 1, yq = yp + 1;
+        if (PERIODIC) {
+          if (ym < 0) ym = ny - 1;
+          if (yq >= ny) yq = 0;
+        }
+        const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
+#pragma unroll
+        for (int i = 0; i < 9; i++) {
+          const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
+          prefetch_l2(Sin + (18 + i) * plane + o, kCopyW * kB);
+        }
+      }
     }
     if (!do2) continue;
 
