@@ -339,3 +339,40 @@ def test_config2_long_run_observables(tlbmod, physics):
         assert umax < 0.3, umax
     for row in log:
         print("config2[%s] step %6d  Nu %.9f  mass_A %.12e  mass_B %.12e  E %.6e  max|uH| %.4e" % ((physics,) + row))
+
+
+def test_distributed_slab_world1_nccl(tlbmod):
+    """The per-rank driver of the multi-GPU path (slabs.DistributedSlab: side stream, events, torch.distributed) with
+    the only process group one GPU allows: world_size 1, NCCL, 127.0.0.1.  A y-periodic lattice makes the single slab
+    its own neighbour across both faces, so pack -> exchange -> unpack all run; the result must equal one handle's."""
+    import os
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_2109_12565_b200 import slabs as S
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK="0", WORLD_SIZE="1")
+    dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda:0"))
+    try:
+        nx, ny = 200, 46
+        par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4, periodic_y=1)
+        solid = (inputs.uniform(8, 9, np.arange(nx * ny)).reshape(ny, nx) < 0.1).astype(np.uint8)
+        rA, rB, T = inputs.smooth_random_fields(nx, ny, 2, 0.5, -0.5)
+        one = tlbmod.TLB(nx, ny, **par)
+        one.set_solid(solid)
+        one.set_fields(rA, rB, T)
+        s = S.DistributedSlab(nx, ny, **par)
+        s.set_solid(solid)
+        s.set_fields(rA, rB, T)
+        one.step(10)
+        s.step(10)
+        torch.cuda.synchronize()
+        for a, b in zip(one.get_populations(), s.t.get_populations()):
+            assert np.array_equal(_np(a), _np(s.owned(b)))
+        ob_1, ob_s = one.observables(), s.observables()
+        for k in ob_1:
+            assert abs(ob_s[k] - ob_1[k]) <= 1e-13 * max(1.0, abs(ob_1[k]))
+    finally:
+        dist.destroy_process_group()
