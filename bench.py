@@ -215,6 +215,32 @@ def run_ours(args, rank, world):
     umax = float((u[0] * u[0] + u[1] * u[1]).max().sqrt())  # print max |u^(H)| of every run
     del u
 
+    # ---- optional: cost of the droplet analysis (section 2.4, first stage) in LB steps; the paper quotes "roughly two LB
+    # time steps" for its whole Delaunay procedure (L218)
+    droplets = None
+    if args.droplets > 0:
+        import ctypes
+        cap = max(1, min(sites // 4, 8 * max(1, cfg["init"]["n_droplets"])))
+        lab = torch.empty((ny, nx), dtype=torch.int32, device=dev)
+        nd = torch.zeros(1, dtype=torch.int32, device=dev)
+        st = torch.zeros((cap, 4), dtype=torch.float64, device=dev)
+        call = lambda: t.lib.tlb_droplets(t.h, ctypes.c_double(args.droplets), lab.data_ptr(), cap, nd.data_ptr(), st.data_ptr())
+        assert call() == 0
+        torch.cuda.synchronize()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(t.stream)
+        for _ in range(20):
+            call()
+        d1.record(t.stream)
+        torch.cuda.synchronize()
+        dms = d0.elapsed_time(d1) / 20
+        k = int(nd.item())
+        droplets = {"B_th": args.droplets, "n_droplets": k, "ms": dms, "lb_steps": dms / step_ms,
+                    "sites_min": float(st[:min(k, cap), 1].min()) if k else None,
+                    "sites_max": float(st[:min(k, cap), 1].max()) if k else None,
+                    "call": "tlb_droplets (fields pass for rho_A, threshold, union-find labelling, flatten, statistics)"}
+        del lab, nd, st
+
     # ---- optional long run with the observables logged (BASELINE config 2: Nu and mass every 1000 steps)
     obs_log = None
     if args.observe_every > 0:
@@ -292,7 +318,7 @@ def run_ours(args, rank, world):
                        if 216 * sites > 4 * 126e6 else "state fits in L2: HBM figures are not meaningful",
                        "parallelism": "1 GPU, whole lattice", "finite": finite, "mass_A": ob["mass_A"], "Nu": ob["Nu"],
                        "max_uH": umax},
-            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_fields": e2e_fields, "observables_log": obs_log,
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "e2e_fields": e2e_fields, "observables_log": obs_log, "droplet_analysis": droplets,
             "gpu_launches": launches, "clocks": clocks,
             "effective_GBs": alg_bytes * mlups / 1e3, "roofline_frac_whole_step": alg_bytes * mlups / 1e3 / peak / world}))
 
@@ -397,6 +423,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--scaling", default="strong", choices=["strong", "weak"],
                     help="N > 1: split the config's lattice into N y-slabs (strong) or stack N copies of it in y (weak)")
+    ap.add_argument("--droplets", type=float, default=0.0,
+                    help="B_th > 0: also time tlb_droplets (threshold B_th on rho_A) on the final state and report it in LB steps")
     ap.add_argument("--observe-every", type=int, default=0,
                     help="also run the config's full step count from its initial state, logging Nu / mass / max|uH| every so many steps")
     ap.add_argument("--pop-precision", type=int, default=64, choices=[64, 32],
