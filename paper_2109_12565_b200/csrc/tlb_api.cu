@@ -16,6 +16,8 @@ struct tlb_handle {
   cudaStream_t st;
   int device;         // CUDA device of the workspace; every entry point runs with it current
   void* S[2];         // population buffers (pull form), 27 planes each, double or float (pop_precision)
+  TMaps maps[2];      // tensor maps of S[0], S[1] (fp64 storage only)
+  bool has_maps;
   double* stage;      // [27][ny][nx] doubles for the *_host population calls when the buffers are float
   double* fld[5];     // rho_A, rho_B, u_x, u_y, T scratch planes
   uint8_t* solid;
@@ -151,8 +153,46 @@ void drop_graphs(tlb_handle* h) {
     if (h->gexec[k]) { cudaGraphExecDestroy(h->gexec[k]); h->gexec[k] = nullptr; }
 }
 
+const TMaps* maps_of(const tlb_handle* h, const void* S) {
+  return h->has_maps ? &h->maps[S == h->S[1] ? 1 : 0] : nullptr;
+}
+
 int launch_step(tlb_handle* h, const void* in, void* out, int ya, int yb, cudaStream_t st) {
-  return launch_fused(h->d, 0, in, out, h->seg_rows, ya, yb, FusedOut{}, st);
+  return launch_fused(h->d, 0, in, out, h->seg_rows, ya, yb, FusedOut{}, maps_of(h, in), st);
+}
+
+// Tensor maps of the two fp64 population buffers (layout: tlb_internal.cuh).  cuTensorMapEncodeTiled is a driver
+// entry point; it is looked up at run time so that the library does not link against libcuda.
+typedef CUresult (*encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool make_maps(tlb_handle* h) {
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  const encode_tiled_fn encode = reinterpret_cast<encode_tiled_fn>(fn);
+  const Dev& d = h->d;
+  const cuuint64_t B = sizeof(double);
+  const cuuint64_t row = (cuuint64_t)d.row * B, plane = (cuuint64_t)d.plane * B;
+  const cuuint64_t dims[5] = {(cuuint64_t)d.px, (cuuint64_t)d.ny + 2, 3, 3, 2};
+  const cuuint64_t strides[4] = {row, plane, 3 * plane - row, 9 * plane};  // bytes, dimensions 1..4
+  const cuuint32_t box[5] = {(cuuint32_t)kCopyW, 1, 3, 3, 2};
+  const cuuint32_t ones[5] = {1, 1, 1, 1, 1};
+  for (int k = 0; k < 2; k++) {
+    char* base = static_cast<char*>(h->S[k]);
+    if (encode(&h->maps[k].f, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+    if (encode(&h->maps[k].g, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base + 18 * plane, dims, strides, box, ones,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  }
+  return true;
 }
 
 // Capture kGraphSteps steps starting from buffer parity `cur` (kernel arguments are baked in: the
@@ -378,6 +418,11 @@ static int create_common(int nx, int ny_glob, int y0, int y1, bool slab, const t
     h->use_graph = false;
   }
   if (configure_kernels() != 0) { cudaGetLastError(); tlb_destroy(h); return TLB_ECUDA; }
+  h->has_maps = false;
+  if (d.prec == 64) {
+    if (!make_maps(h)) { tlb_destroy(h); return TLB_ECUDA; }  // no second code path: fail loudly
+    h->has_maps = true;
+  }
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
   cu(h, cudaMemsetAsync(h->count, 0, sizeof(int), h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field
@@ -640,7 +685,7 @@ int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundar
 // rows the non-stepping modes of the fused kernel sweep: the owned ones
 static int fused_mode(tlb_handle* h, int mode, const FusedOut& out) {
   const int seg = default_seg_rows(h->d.nx, h->d.own1 - h->d.own0);
-  h->launches += launch_fused(h->d, mode, h->S[h->cur], nullptr, seg, h->d.own0, h->d.own1, out, h->st);
+  h->launches += launch_fused(h->d, mode, h->S[h->cur], nullptr, seg, h->d.own0, h->d.own1, out, maps_of(h, h->S[h->cur]), h->st);
   return check(h);
 }
 

@@ -44,9 +44,9 @@ __global__ void scatter_kernel(const Dev d, const double* __restrict__ a, const 
         va = a[i * n + q]; vb = b[i * n + q]; vc = c[i * n + q];
       }
     }
-    S[i * d.plane + o] = (ST)va;
-    S[(9 + i) * d.plane + o] = (ST)vb;
-    S[(18 + i) * d.plane + o] = (ST)vc;
+    S[pslot(i) * d.plane + o] = (ST)va;
+    S[(9 + pslot(i)) * d.plane + o] = (ST)vb;
+    S[(18 + pslot(i)) * d.plane + o] = (ST)vc;
   }
 }
 
@@ -66,9 +66,9 @@ __global__ void gather_kernel(const Dev d, const ST* __restrict__ S, double* __r
     int sy = y - cy(i);
     if (d.periodic_y) sy = wrapi(sy, ny);
     const long long o = d.at(sx, sy);
-    if (a) a[i * n + q] = sol ? 0.0 : (double)S[i * d.plane + o];
-    if (b) b[i * n + q] = sol ? 0.0 : (double)S[(9 + i) * d.plane + o];
-    if (c) c[i * n + q] = sol ? 0.0 : (double)S[(18 + i) * d.plane + o];
+    if (a) a[i * n + q] = sol ? 0.0 : (double)S[pslot(i) * d.plane + o];
+    if (b) b[i * n + q] = sol ? 0.0 : (double)S[(9 + pslot(i)) * d.plane + o];
+    if (c) c[i * n + q] = sol ? 0.0 : (double)S[(18 + pslot(i)) * d.plane + o];
   }
 }
 

@@ -14,9 +14,13 @@
 //     writes its images, so no separate halo-refresh pass exists.
 // A plane is [ny + 2][px] doubles, x fastest, lattice column x at offset kXL + x within a row; px
 // and kXL are multiples of 16 doubles so that x = 0 of every row starts a 128-byte line and the
-// strip copies of the fused kernel (cp.async.bulk) are 16-byte aligned.  27 planes per buffer:
-// [0, 9) f_A, [9, 18) f_B, [18, 27) g, direction order R1.
+// strip copies of the fused kernel are 16-byte aligned.  27 planes per buffer: [0, 9) f_A, [9, 18) f_B,
+// [18, 27) g; inside a set the planes are ordered by c_y (pslot() below): the three directions with
+// c_y = -1, then c_y = 0, then c_y = +1.  A target row r pulls storage row (r + 1) - c_y of plane i, so
+// with this order ONE tensor-map copy (cp.async.bulk.tensor, box x * 1 row * 3 planes * 3 groups * 2 species,
+// group stride = 3 planes - 1 row) brings the 18 fluid plane rows of a strip, already shifted in y.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -28,6 +32,10 @@ namespace tlb {
 __host__ __device__ constexpr int cx(int i) { return i == 1 || i == 5 || i == 8 ? 1 : (i == 3 || i == 6 || i == 7 ? -1 : 0); }
 __host__ __device__ constexpr int cy(int i) { return i == 2 || i == 5 || i == 6 ? 1 : (i == 4 || i == 7 || i == 8 ? -1 : 0); }
 __host__ __device__ constexpr int opp(int i) { return i == 0 ? 0 : (i <= 4 ? ((i + 1) % 4) + 1 : ((i - 3) % 4) + 5); }
+// plane of direction i inside its set (internal order, see above); the ABI keeps the order R1
+__host__ __device__ constexpr int pslot(int i) {
+  return i == 4 ? 0 : i == 7 ? 1 : i == 8 ? 2 : i == 0 ? 3 : i == 1 ? 4 : i == 3 ? 5 : i == 2 ? 6 : i == 5 ? 7 : 8;
+}
 __host__ __device__ constexpr double wq(int i) { return i == 0 ? 4.0 / 9.0 : (i <= 4 ? 1.0 / 9.0 : 1.0 / 36.0); }
 
 // fused-kernel geometry (see tlb_step.cu)
@@ -85,9 +93,18 @@ struct FusedOut {
   double* partials;                   // MODE 3: [CTAs][6] {mass_A, mass_B, sum |u|^2, sum u_y T, sum d_y T, fluid sites}
 };
 
+// Tensor maps of one fp64 population buffer (built by tlb_create with cuTensorMapEncodeTiled):
+//   f: 5-D (x, row, plane-in-group 3, c_y group 3, species 2), strides (1, row, plane, 3 plane - row, 9 plane);
+//   g: 4-D, the same without the species dimension, based at plane 18.
+// Row coordinate r + 2 addresses, in group k (c_y = k - 1), storage row r + 2 - k = (r + 1) - c_y.
+struct TMaps {
+  CUtensorMap f, g;
+};
+
 // launchers (each returns the number of kernels it launched)
+// maps: the tensor maps of the buffer Sin (fp64 storage), or null (fp32 storage: 1-D bulk copies)
 int launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
-                 cudaStream_t st);
+                 const TMaps* maps, cudaStream_t st);
 int fused_grid_ctas(const Dev& d, int seg_rows, int rows);  // CTAs launch_fused uses for `rows` rows
 int launch_boundary(const Dev& d, void* S, const int* sites, int n_sites, cudaStream_t st);
 int launch_build_links(const Dev& d, int* sites, int* count, uint8_t* solidp, cudaStream_t st);

@@ -3,10 +3,12 @@
 //
 // Fused kernel, "strip marching with an asynchronous row pipeline".  A CTA of 2 kW threads (two per
 // lattice column, one per species) owns kW columns and marches over a segment of rows.  For every row r one elected thread issues
-// 18 bulk asynchronous copies (cp.async.bulk, the 1-D TMA path; SASS UBLKCP) that bring the strip
-// of the 18 fluid planes, already shifted in y by the pull rule f_i(x, r) = S_i(x - c_i), into a
-// 4-slot ring in shared memory and complete on an mbarrier; the x shift is applied when threads
-// read the ring.  Each landed row is used twice without touching HBM or L2 again:
+// ONE tensor-map copy (cp.async.bulk.tensor.5d, TMA; SASS UTMALDG) whose box holds the strip of all 18 fluid
+// planes, each already shifted in y by the pull rule f_i(x, r) = S_i(x - c_i) (the planes are stored in c_y
+// order so that the shift is a stride of the tensor map, tlb_internal.cuh), into a 4-slot ring in shared
+// memory, completing on an mbarrier; the x shift is applied when threads read the ring.  (fp32 storage and the
+// two wrap rows of a y-periodic lattice use 18 1-D bulk copies, SASS UBLKCP, instead.)  Each landed row is
+// used twice without touching HBM or L2 again:
 //   (1) when it lands: rho_A, rho_B (Eq. (4)) and psi^s (Eq. (12)) of row r for the strip plus its
 //       2-cell halo go into a 6-row ring {rho_A, rho_B, psi^s_A, psi^s_B};
 //   (2) two rows later, with stencil rows y-2..y+2 resident: 5x5 force stencils (Eqs. (7), (10),
@@ -65,6 +67,21 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
           smem_u32(dst)),
       "l"(__cvta_generic_to_global(src)), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
+}
+// tensor-map copy (TMA, SASS UTMALDG) of the box at coordinates (c0 .. c4) of a 5-D map, completing on `bar`
+__device__ __forceinline__ void tma_g2s_5d(void* dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, int c4,
+                                           uint64_t* bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4, %5, %6}], [%7], %8;" ::"r"(smem_u32(dst)),
+      "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4), "r"(smem_u32(bar)), "l"(policy)
+      : "memory");
+}
+// L2 prefetch of the box at (c0 .. c3) of a 4-D map (SASS UTMAPF)
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];" ::"l"(map), "r"(c0), "r"(c1),
+               "r"(c2), "r"(c3)
+               : "memory");
 }
 // L2 prefetch of `bytes` (multiple of 16, 16-byte aligned): starts the HBM read rows ahead of the loads that use it
 __device__ __forceinline__ void prefetch_l2(const void* src, uint32_t bytes) {
@@ -127,8 +144,9 @@ __device__ __forceinline__ int wrap_row(int r, int ny) {
 }
 
 // The thermal populations reach the lanes through plain loads issued in the iteration that uses them, so their
-// latency is exposed unless the lines are already in L2: the warp that re-arms a slot also prefetches the 9 thermal
-// plane rows of the row that reaches phase 2 kGPrefetchRows iterations later (measured on config 4, same box:
+// latency is exposed unless the lines are already in L2: the warp that re-arms a slot also prefetches (one
+// cp.async.bulk.prefetch.tensor.4d, SASS UTMAPF) the 9 thermal plane rows of the row that reaches phase 2
+// kGPrefetchRows iterations later (measured on config 4, same box:
 // 0.717 ms without, 0.724 / 0.695 / 0.684 / 0.682 / 0.684 / 0.690 / 0.714 ms at 1 / 2 / 3 / 4 / 6 / 8 / 12 rows;
 // prefetching the 18 fluid plane rows as well costs 5 %: the bulk copies already run a row and a half ahead).
 constexpr int kGPrefetchRows = 4;
@@ -185,7 +203,8 @@ __device__ __forceinline__ double relax_tau1(double owd, double cu, double usq) 
 template <int MODE, bool PERIODIC, typename ST>
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
 fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int seg_rows, int ya, int yb,
-             const FusedOut out) {
+             const FusedOut out, const __grid_constant__ TMaps tm) {
+  constexpr bool kTensor = sizeof(ST) == 8;  // fp64 storage: tensor-map copies; fp32 (bandwidth study): 1-D bulk copies
   double* __restrict__ const oRA = out.rhoA;
   double* __restrict__ const oRB = out.rhoB;
   double* __restrict__ const oUx = out.ux;
@@ -229,13 +248,18 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     }
     uint64_t* bar = &sm.full[q & 3];
     mbar_expect_tx(bar, 18u * kCopyW * kB);
+    if (kTensor && (!PERIODIC || (rr > 0 && rr < ny - 1))) {
+      // one copy: box 136 x 1 x 3 x 3 x 2 = the 18 fluid plane rows, each shifted by its c_y (tlb_internal.cuh)
+      tma_g2s_5d(&sm.f[q & 3][0][0], &tm.f, kXL + x0 - kHX, rr + 2, 0, 0, 0, bar, pol);
+      return;
+    }
     const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
 #pragma unroll
     for (int l = 0; l < 2; l++)
 #pragma unroll
       for (int i = 0; i < 9; i++) {
         const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-        bulk_g2s(&sm.f[q & 3][l * 9 + i][0], Sin + (l * 9 + i) * plane + o, kCopyW * kB, bar, pol);
+        bulk_g2s(&sm.f[q & 3][l * 9 + pslot(i)][0], Sin + (l * 9 + pslot(i)) * plane + o, kCopyW * kB, bar, pol);
       }
   };
   if (t == 0) {
@@ -265,9 +289,12 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
   const double sgn = s ? -1.0 : 1.0;                  // this lane's thermal directions are sgn * {c_1, c_2, c_5, c_6}
 
   // running byte pointers of row y = y0 (advanced by one row per phase-2 iteration)
-  const char* gp = reinterpret_cast<const char*>(Sin + (18 + 2 * s) * plane + d.at(x, y0));   // g_{i + 2s}
+  // thermal planes of lane s (internal order pslot()): g_0 at plane 3 (lane 0 only), g_1 / g_3 at 4 + s,
+  // {g_2, g_5, g_6} at 6, 7, 8 (lane 0), {g_4, g_7, g_8} at 0, 1, 2 (lane 1): 6 planes lower
+  const char* gp = reinterpret_cast<const char*>(Sin + (18 + s) * plane + d.at(x, y0));
   char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + d.at(x, y0));                    // own species
-  char* opg = reinterpret_cast<char*>(Sout + (18 + 2 * s) * plane + d.at(x, y0));             // own thermal half
+  char* opg = reinterpret_cast<char*>(Sout + (18 + s) * plane + d.at(x, y0));                 // own thermal half
+  const long long sofs = s ? -7 * planeB : 0;                                                    // planes 6.. -> 0.. for lane 1
   const int co = s ? kB : -kB;                                                                    // x - c_x of c_1 / c_3
 
   // thermal populations of (x, y).  Lane s = 0 reads
@@ -280,11 +307,12 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       if (!s && y == 0) rofs = (long long)(ny - 1) * rowB;
       if (s && y == ny - 1) rofs = -(long long)(ny - 1) * rowB;
     }
-    g0 = ldg_stream(reinterpret_cast<const ST*>(gp - (s ? 2 * planeB : 0)), pol);
-    ga = ldg_stream(reinterpret_cast<const ST*>(gp + 1 * planeB + co), pol);
-    gb = ldg_stream(reinterpret_cast<const ST*>(gp + 2 * planeB + rofs), pol);
-    gc = ldg_stream(reinterpret_cast<const ST*>(gp + 5 * planeB + rofs + co), pol);
-    gd = ldg_stream(reinterpret_cast<const ST*>(gp + 6 * planeB + rofs - co), pol);
+    rofs += sofs;
+    g0 = ldg_stream(reinterpret_cast<const ST*>(gp + 3 * planeB), pol);  // lane 1 reads g_1 here and never uses it
+    ga = ldg_stream(reinterpret_cast<const ST*>(gp + 4 * planeB + co), pol);
+    gb = ldg_stream(reinterpret_cast<const ST*>(gp + 6 * planeB + rofs), pol);
+    gc = ldg_stream(reinterpret_cast<const ST*>(gp + 7 * planeB + rofs + co), pol);
+    gd = ldg_stream(reinterpret_cast<const ST*>(gp + 8 * planeB + rofs - co), pol);
   };
 
   uint32_t parity = 0;  // one bit per slot
@@ -315,7 +343,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
         const ST* fs = &sm.f[slot][9 * s][kWC * wid + c + 2];  // S(x) of ring column c
         double f[9];
 #pragma unroll
-        for (int i = 0; i < 9; i++) f[i] = (double)fs[i * kSW - cx(i)];
+        for (int i = 0; i < 9; i++) f[i] = (double)fs[pslot(i) * kSW - cx(i)];
         rl = sum9(f);
         pl = d.rho0 * (1.0 - exp_nonpos(-rl * d.inv_rho0));
       }
@@ -329,7 +357,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     {
       const ST* fs = &sm.f[slot2][9 * s][kWC * wid + k + kHX];
 #pragma unroll
-      for (int i = 0; i < 9; i++) f[i] = (double)fs[i * kSW - cx(i)];
+      for (int i = 0; i < 9; i++) f[i] = (double)fs[pslot(i) * kSW - cx(i)];
     }
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
     if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1) {  // last warp out: the slot is free
@@ -341,11 +369,15 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
           if (ym < 0) ym = ny - 1;
           if (yq >= ny) yq = 0;
         }
-        const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
+        if (kTensor && (!PERIODIC || (yp > 0 && yp < ny - 1))) {
+          tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp + 2, 0, 0);
+        } else {
+          const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
 #pragma unroll
-        for (int i = 0; i < 9; i++) {
-          const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-          prefetch_l2(Sin + (18 + i) * plane + o, kCopyW * kB);
+          for (int i = 0; i < 9; i++) {
+            const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
+            prefetch_l2(Sin + (18 + pslot(i)) * plane + o, kCopyW * kB);
+          }
         }
       }
     }
@@ -504,26 +536,26 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       }
       if (MODE == 0 && fluid) {
 #pragma unroll
-        for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<ST*>(opf + i * planeB), f[i], pol);
+        for (int i = 0; i < 9; i++) stg_stream(reinterpret_cast<ST*>(opf + pslot(i) * planeB), f[i], pol);
         if (d.thermal) {
-          if (!s) stg_stream(reinterpret_cast<ST*>(opg), g0, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 1 * planeB), ga, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 2 * planeB), gb, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 5 * planeB), gc, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 6 * planeB), gd, pol);
+          if (!s) stg_stream(reinterpret_cast<ST*>(opg + 3 * planeB), g0, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 4 * planeB), ga, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 6 * planeB + sofs), gb, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 7 * planeB + sofs), gc, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 8 * planeB + sofs), gd, pol);
         }
         if (x < kGhost || x >= nx - kGhost) {  // periodic images of this column (ghost columns)
           for (int pass = 0; pass < 2; pass++)
             for (int xg = pass ? x - nx : x + nx; pass ? xg >= -kGhost : xg < nx + kGhost; xg += pass ? -nx : nx) {
               const long long e = (long long)(xg - x) * kB;
 #pragma unroll
-              for (int i = 0; i < 9; i++) *reinterpret_cast<ST*>(opf + i * planeB + e) = (ST)f[i];
+              for (int i = 0; i < 9; i++) *reinterpret_cast<ST*>(opf + pslot(i) * planeB + e) = (ST)f[i];
               if (d.thermal) {
-                if (!s) *reinterpret_cast<ST*>(opg + e) = (ST)g0;
-                *reinterpret_cast<ST*>(opg + 1 * planeB + e) = (ST)ga;
-                *reinterpret_cast<ST*>(opg + 2 * planeB + e) = (ST)gb;
-                *reinterpret_cast<ST*>(opg + 5 * planeB + e) = (ST)gc;
-                *reinterpret_cast<ST*>(opg + 6 * planeB + e) = (ST)gd;
+                if (!s) *reinterpret_cast<ST*>(opg + 3 * planeB + e) = (ST)g0;
+                *reinterpret_cast<ST*>(opg + 4 * planeB + e) = (ST)ga;
+                *reinterpret_cast<ST*>(opg + 6 * planeB + sofs + e) = (ST)gb;
+                *reinterpret_cast<ST*>(opg + 7 * planeB + sofs + e) = (ST)gc;
+                *reinterpret_cast<ST*>(opg + 8 * planeB + sofs + e) = (ST)gd;
               }
             }
         }
@@ -592,7 +624,8 @@ boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, 
   const long long plane = d.plane;
   const long long os = d.at(sx, sy), ox = d.at(x, y);
   const int io = opp(i);
-  ST va = S[io * plane + ox], vb = S[(9 + io) * plane + ox];
+  const int pi = pslot(i), po = pslot(io);
+  ST va = S[po * plane + ox], vb = S[(9 + po) * plane + ox];
   // R20: a moving flat wall (ghost row, not a post) hands the population back with the wall's momentum,
   // f_i = f*_opp(i) + 2 w_i rho_l (c_i . u_w) / c_s^2; rho_l(x) = sum_j S_l,j(x) (collision conserves it)
   const double uw = sy < 0 ? d.u_wall_bottom : (sy >= ny ? d.u_wall_top : 0.0);
@@ -603,16 +636,16 @@ boundary_kernel(const Dev d, ST* __restrict__ S, const int* __restrict__ sites, 
     va = (ST)((double)va + 6.0 * wq(i) * ra * (cx(i) * uw));
     vb = (ST)((double)vb + 6.0 * wq(i) * rb * (cx(i) * uw));
   }
-  const ST vg = d.thermal ? (ST)(-(double)S[(18 + io) * plane + ox] + 2.0 * wq(i) * Tw) : (ST)0;
+  const ST vg = d.thermal ? (ST)(-(double)S[(18 + po) * plane + ox] + 2.0 * wq(i) * Tw) : (ST)0;
   for (int xg = sx; xg < nx + kGhost; xg += nx) {  // the node and its right-hand images
-    S[i * plane + os + (xg - sx)] = va;
-    S[(9 + i) * plane + os + (xg - sx)] = vb;
-    if (d.thermal) S[(18 + i) * plane + os + (xg - sx)] = vg;
+    S[pi * plane + os + (xg - sx)] = va;
+    S[(9 + pi) * plane + os + (xg - sx)] = vb;
+    if (d.thermal) S[(18 + pi) * plane + os + (xg - sx)] = vg;
   }
   for (int xg = sx - nx; xg >= -kGhost; xg -= nx) {
-    S[i * plane + os + (xg - sx)] = va;
-    S[(9 + i) * plane + os + (xg - sx)] = vb;
-    if (d.thermal) S[(18 + i) * plane + os + (xg - sx)] = vg;
+    S[pi * plane + os + (xg - sx)] = va;
+    S[(9 + pi) * plane + os + (xg - sx)] = vb;
+    if (d.thermal) S[(18 + pi) * plane + os + (xg - sx)] = vg;
   }
 }
 
@@ -671,27 +704,29 @@ int fused_grid_ctas(const Dev& d, int seg_rows, int rows) {
 
 template <int MODE, typename ST>
 static void launch_mode(const Dev& d, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
-                        cudaStream_t st) {
+                        const TMaps& tm, cudaStream_t st) {
   const ST* in = static_cast<const ST*>(Sin);
   ST* o = static_cast<ST*>(Sout);
   const dim3 g = strip_grid(d, seg_rows, yb - ya);
   const size_t sm = sizeof(Smem<ST>);
-  if (d.periodic_y) fused_kernel<MODE, true, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out);
-  else fused_kernel<MODE, false, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out);
+  if (d.periodic_y) fused_kernel<MODE, true, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
+  else fused_kernel<MODE, false, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
 }
 
 // Launch the fused kernel in `mode` on local rows [ya, yb); returns the number of launches (0 for an empty range).
 int launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
-                 cudaStream_t st) {
+                 const TMaps* maps, cudaStream_t st) {
   if (yb <= ya) return 0;
+  static const TMaps none{};  // fp32 storage never reads the maps
+  const TMaps& tm = maps ? *maps : none;
   if (seg_rows > yb - ya) seg_rows = yb - ya;
   if (seg_rows < 1) seg_rows = 1;
   const bool f32 = d.prec == 32;
   switch (mode) {
-    case 0: f32 ? launch_mode<0, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<0, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
-    case 1: f32 ? launch_mode<1, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<1, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
-    case 2: f32 ? launch_mode<2, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<2, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
-    default: f32 ? launch_mode<3, float>(d, Sin, Sout, seg_rows, ya, yb, out, st) : launch_mode<3, double>(d, Sin, Sout, seg_rows, ya, yb, out, st); break;
+    case 0: f32 ? launch_mode<0, float>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st) : launch_mode<0, double>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st); break;
+    case 1: f32 ? launch_mode<1, float>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st) : launch_mode<1, double>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st); break;
+    case 2: f32 ? launch_mode<2, float>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st) : launch_mode<2, double>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st); break;
+    default: f32 ? launch_mode<3, float>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st) : launch_mode<3, double>(d, Sin, Sout, seg_rows, ya, yb, out, tm, st); break;
   }
   return 1;
 }
