@@ -10,7 +10,7 @@
  *
  * The method is an explicit iteration, so the oracle follows it step by step in the
  * paper's order and notation (PAPER Eqs. (1)-(22)); readings of silent / garbled passages
- * are the ones listed in DESIGN.md ("Readings R1..R22").  No blocking, fusion or reordering:
+ * are the ones listed in DESIGN.md ("Readings R1..R26").  No blocking, fusion or reordering:
  * every sub-step is a full sweep over the lattice writing a full array.
  *
  * Parity pins (tests/test_oracle_pins.py, all run with -m "not gpu"):
@@ -32,6 +32,11 @@
  *                      (all couplings)                                       L248-250, L294-296, Eq. (14) (R21)
  *   droplets           hand-made masks with known clusters, a droplet across the x seam, exact centroids of
  *                      discs, invariance under x shifts                      section 2.4 L198 (R22)
+ *   Voronoi / Delaunay half planes, rectangular cells and ties by hand; the defining minimum property checked in numpy;
+ *   / T1 / Nu_drop     links equal to the continuum Delaunay triangulation (scipy.spatial, periodic images and
+ *                      wall mirror images) of jittered triangular arrangements; a hand-made diagonal flip and
+ *                      flips of a triangulated grid; Nu_drop = 1 + U T(y_i) ny / (kappa dT) in a uniform stream
+ *                      (tests/test_oracle_analysis.py)               section 2.4, Eq. (25) (R23-R26)
  *   posts / corners    second, independently written streaming formulation
  *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
  *                      pull of orc_step; beyond that and mass conservation the post-corner
@@ -580,6 +585,174 @@ int orc_droplets(orc_state *s, double B_th, int32_t *labels, int max_droplets, d
   free(stack);
   if (!labels) free(lab);
   return found;
+}
+
+/* ---- Droplet analysis, second stage (section 2.4; readings R23-R26 of DESIGN.md).  The paper gives the
+ * ingredients in prose and defers the details to its ref. [58], which is not available; every choice below is a
+ * reading.  These functions are geometric: they take the centres / colours / link lists as arguments. ---- */
+
+/* signed offset a - c for a lattice coordinate a and a real centre coordinate c, minimum image when periodic */
+static double offset_to(int a, double c, int n, int periodic) {
+  double d = (double)a - c;
+  if (periodic) {
+    const double half = 0.5 * (double)n;
+    if (d > half) d -= (double)n;
+    else if (d < -half) d += (double)n;
+  }
+  return d;
+}
+
+/* R23, digital Voronoi tessellation (L198: "each point of the lattice is coloured by the label of the nearest centre
+ * of mass"): colour[y][x] = index k of the centre with the smallest squared distance dx*dx + dy*dy (fp64, x minimum
+ * image, y minimum image iff periodic_y); ties go to the smallest index; -1 when there are no centres.  Brute force. */
+void orc_voronoi(int nx, int ny, int periodic_y, const double *centres, int n, int32_t *colour) {
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      int best = -1;
+      double bd = 0.0;
+      for (int k = 0; k < n; k++) {
+        const double dx = offset_to(x, centres[2 * k], nx, 1), dy = offset_to(y, centres[2 * k + 1], ny, periodic_y);
+        const double d2 = dx * dx + dy * dy;
+        if (best < 0 || d2 < bd) { best = k; bd = d2; }
+      }
+      colour[(size_t)y * nx + x] = best;
+    }
+}
+
+static int cmp_pair(const void *a, const void *b) {
+  const int32_t *p = (const int32_t *)a, *q = (const int32_t *)b;
+  if (p[0] != q[0]) return p[0] < q[0] ? -1 : 1;
+  if (p[1] != q[1]) return p[1] < q[1] ? -1 : 1;
+  return 0;
+}
+static int sort_unique_pairs(int32_t *v, int n) {
+  qsort(v, (size_t)n, 2 * sizeof(int32_t), cmp_pair);
+  int m = 0;
+  for (int k = 0; k < n; k++)
+    if (m == 0 || v[2 * k] != v[2 * m - 2] || v[2 * k + 1] != v[2 * m - 1]) { v[2 * m] = v[2 * k]; v[2 * m + 1] = v[2 * k + 1]; m++; }
+  return m;
+}
+
+/* R24, Delaunay links (L198: "The vertices at which adjacent digital Voronoi cells converge are used to identify the
+ * Delaunay triangulation").  A vertex is a 2 x 2 block of lattice sites {(x, y), (x+1, y), (x, y+1), (x+1, y+1)}
+ * (x periodic; y periodic iff periodic_y, else the rows y = -1 and y = ny beyond the flat walls carry the wall
+ * colour -1, so that a Voronoi edge that ends on a wall still ends in a vertex) that holds at least 3 distinct
+ * colours.  Three colours: every pair of droplet colours in the block is a link.  Four colours (the degenerate
+ * quadrilateral): the four side-adjacent pairs and the pair on the main diagonal (x, y)-(x+1, y+1).
+ * Output: the distinct links (a < b) in lexicographic order; returns their number, writes at most max_links. */
+int orc_delaunay(int nx, int ny, int periodic_y, const int32_t *colour, int max_links, int32_t *links) {
+  int cap = 1024, n = 0;
+  int32_t *v = (int32_t *)malloc((size_t)cap * 2 * sizeof(int32_t));
+  for (int y = periodic_y ? 0 : -1; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      const int x1 = x + 1 == nx ? 0 : x + 1;
+      int y1 = y + 1;
+      if (periodic_y && y1 == ny) y1 = 0;
+      const int32_t c00 = y < 0 ? -1 : colour[(size_t)y * nx + x], c10 = y < 0 ? -1 : colour[(size_t)y * nx + x1];
+      const int32_t c01 = y1 >= ny ? -1 : colour[(size_t)y1 * nx + x], c11 = y1 >= ny ? -1 : colour[(size_t)y1 * nx + x1];
+      const int32_t c[4] = {c00, c10, c01, c11};
+      int distinct = 0;
+      for (int i = 0; i < 4; i++) {
+        int seen = 0;
+        for (int j = 0; j < i; j++) seen |= c[j] == c[i];
+        distinct += !seen;
+      }
+      if (distinct < 3) continue;
+      /* pairs of block positions: sides 0-1, 2-3, 0-2, 1-3, diagonals 0-3 (main), 1-2 */
+      static const int PA[6] = {0, 2, 0, 1, 0, 1}, PB[6] = {1, 3, 2, 3, 3, 2};
+      for (int e = 0; e < 6; e++) {
+        if (distinct == 4 && e == 5) continue;
+        int32_t a = c[PA[e]], b = c[PB[e]];
+        if (a < 0 || b < 0 || a == b) continue;
+        if (a > b) { const int32_t t = a; a = b; b = t; }
+        if (n == cap) { cap *= 2; v = (int32_t *)realloc(v, (size_t)cap * 2 * sizeof(int32_t)); }
+        v[2 * n] = a; v[2 * n + 1] = b; n++;
+      }
+    }
+  n = sort_unique_pairs(v, n);
+  for (int k = 0; k < n && k < max_links; k++) { links[2 * k] = v[2 * k]; links[2 * k + 1] = v[2 * k + 1]; }
+  free(v);
+  return n;
+}
+
+/* R25 (first half), droplet identity between two frames: droplet i of the present frame is the droplet of the past
+ * frame in whose digital Voronoi cell its centre lies, map[i] = colour_past at the lattice site nearest to the
+ * centre (floor(c + 1/2), x wrapped, y wrapped or clamped). */
+static int nearest_site(double c, int n, int periodic) {
+  int r = (int)floor(c + 0.5);
+  if (periodic) { r %= n; if (r < 0) r += n; }
+  else { if (r < 0) r = 0; if (r >= n) r = n - 1; }
+  return r;
+}
+void orc_match(int nx, int ny, int periodic_y, const int32_t *colour_past, const double *centres_now, int n_now, int32_t *map) {
+  for (int i = 0; i < n_now; i++)
+    map[i] = colour_past[(size_t)nearest_site(centres_now[2 * i + 1], ny, periodic_y) * nx + nearest_site(centres_now[2 * i], nx, 1)];
+}
+
+static int has_pair(const int32_t *v, int n, int32_t a, int32_t b) {
+  if (a > b) { const int32_t t = a; a = b; b = t; }
+  for (int k = 0; k < n; k++)
+    if (v[2 * k] == a && v[2 * k + 1] == b) return 1;
+  return 0;
+}
+
+/* R25 (second half), T1 events (L198-200: "Subsequent Delaunay triangulations are compared in order to detect T1
+ * plastic rearrangements ... These topological events only involve 4 droplets ... at the four vertices of a
+ * quadrilateral labelled a, b, c and d, and they are associated with a 'flip' of the diagonal link": "the diagonal
+ * link between a and b is replaced by the link between c and d").  The links of the present frame are first written
+ * in the indices of the past frame through `map` (links with an unmatched end, map < 0, or with both ends on the same
+ * past droplet are dropped).  An event (a, b, c, d), a < b, c < d, is: link a-b in the past and not now; link c-d now
+ * and not in the past; the four sides a-c, a-d, b-c, b-d present in both frames.  Plain search over all quadruples
+ * of links; output in lexicographic order; returns the number of events, writes at most max_events. */
+int orc_t1_events(const int32_t *past, int n_past, const int32_t *now, int n_now, const int32_t *map, int max_events,
+                  int32_t *events) {
+  int32_t *cur = (int32_t *)malloc((size_t)(n_now > 0 ? n_now : 1) * 2 * sizeof(int32_t));
+  int m = 0;
+  for (int k = 0; k < n_now; k++) {
+    int32_t a = map ? map[now[2 * k]] : now[2 * k], b = map ? map[now[2 * k + 1]] : now[2 * k + 1];
+    if (a < 0 || b < 0 || a == b) continue;
+    if (a > b) { const int32_t t = a; a = b; b = t; }
+    cur[2 * m] = a; cur[2 * m + 1] = b; m++;
+  }
+  m = sort_unique_pairs(cur, m);
+  int found = 0;
+  for (int k = 0; k < n_past; k++) {          /* past links in lexicographic order -> events come out sorted by (a, b) */
+    const int32_t a = past[2 * k], b = past[2 * k + 1];
+    if (has_pair(cur, m, a, b)) continue;
+    for (int j = 0; j < m; j++) {             /* present links in lexicographic order -> then by (c, d) */
+      const int32_t c = cur[2 * j], d = cur[2 * j + 1];
+      if (has_pair(past, n_past, c, d)) continue;
+      if (c == a || c == b || d == a || d == b) continue;
+      const int sides = has_pair(past, n_past, a, c) && has_pair(past, n_past, a, d) && has_pair(past, n_past, b, c) &&
+                        has_pair(past, n_past, b, d) && has_pair(cur, m, a, c) && has_pair(cur, m, a, d) &&
+                        has_pair(cur, m, b, c) && has_pair(cur, m, b, d);
+      if (!sides) continue;
+      if (found < max_events) { events[4 * found] = a; events[4 * found + 1] = b; events[4 * found + 2] = c; events[4 * found + 3] = d; }
+      found++;
+    }
+  }
+  free(cur);
+  return found;
+}
+
+/* R26, droplet Nusselt number, Eq. (25): Nu_i = [u_y T - kappa d_y T](X_i) / (kappa dT / ny) with the fields
+ * "evaluated for the i-th droplet" read at the lattice site nearest to its centre X_i: u_y = u_y^(H), kappa and d_y T as
+ * in Eq. (24) / R10; 0 if that site is solid or dT = 0. */
+void orc_droplet_nusselt(orc_state *s, const double *centres, int n, double *nu) {
+  const int nx = s->nx, ny = s->ny;
+  moments_and_forces(s);
+  const double kappa = (s->p.tau_g - 0.5) / 3.0, DT = s->p.T_bottom - s->p.T_top;
+  for (int i = 0; i < n; i++) {
+    const int x = nearest_site(centres[2 * i], nx, 1), y = nearest_site(centres[2 * i + 1], ny, s->p.periodic_y);
+    const size_t k = IDX(s, x, y);
+    if (s->solid[k] || DT == 0.0) { nu[i] = 0.0; continue; }
+    double up, dn;
+    if (is_solid(s, x, y + 1)) up = T_wall(s, s->p.periodic_y ? wrap(y + 1, ny) : y + 1);
+    else up = 0.5 * (s->T[k] + s->T[IDX(s, x, s->p.periodic_y ? wrap(y + 1, ny) : y + 1)]);
+    if (is_solid(s, x, y - 1)) dn = T_wall(s, s->p.periodic_y ? wrap(y - 1, ny) : y - 1);
+    else dn = 0.5 * (s->T[k] + s->T[IDX(s, x, s->p.periodic_y ? wrap(y - 1, ny) : y - 1)]);
+    nu[i] = (s->uHy[k] * s->T[k] - kappa * (up - dn)) / (kappa * DT / ny);
+  }
 }
 
 /* lattice constants exported for the weight-invariant pins */

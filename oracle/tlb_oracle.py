@@ -59,6 +59,14 @@ def _load():
         lib.orc_row_momentum_x.argtypes = [ctypes.c_void_p, dp]
         lib.orc_droplets.restype = ctypes.c_int
         lib.orc_droplets.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p, ctypes.c_int, dp]
+        i32p = ctypes.c_void_p
+        lib.orc_voronoi.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_int, i32p]
+        lib.orc_delaunay.restype = ctypes.c_int
+        lib.orc_delaunay.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, ctypes.c_int, i32p]
+        lib.orc_match.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, dp, ctypes.c_int, i32p]
+        lib.orc_t1_events.restype = ctypes.c_int
+        lib.orc_t1_events.argtypes = [i32p, ctypes.c_int, i32p, ctypes.c_int, i32p, ctypes.c_int, i32p]
+        lib.orc_droplet_nusselt.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp]
         lib.orc_w.restype = ctypes.c_double
         lib.orc_w.argtypes = [ctypes.c_int, ctypes.c_int]
         lib.orc_p.restype = ctypes.c_double
@@ -188,6 +196,59 @@ Oracle.stress_xy = _stress_xy
 Oracle.x_average_stress = _x_average_stress
 Oracle.row_momentum_x = _row_momentum_x
 Oracle.droplets = _droplets
+
+
+def _droplet_nusselt(self, centres):
+    """Nu_i of Eq. (25) at the lattice site nearest to each centre [n][2] (reading R26)."""
+    c = _c(centres).reshape(-1, 2)
+    nu = np.zeros(len(c))
+    self.lib.orc_droplet_nusselt(self.h, _dp(c), len(c), _dp(nu))
+    return nu
+
+
+Oracle.droplet_nusselt = _droplet_nusselt
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def voronoi(nx, ny, periodic_y, centres):
+    """Digital Voronoi colouring [ny][nx] int32 of the centres [n][2] (reading R23); brute force."""
+    c = _c(centres).reshape(-1, 2)
+    colour = np.zeros((ny, nx), dtype=np.int32)
+    _load().orc_voronoi(int(nx), int(ny), int(bool(periodic_y)), _dp(c), len(c), colour.ctypes.data)
+    return colour
+
+
+def delaunay(colour, periodic_y, max_links=None):
+    """Sorted distinct Delaunay links [m][2] of a colouring (reading R24)."""
+    colour = _i32(colour)
+    ny, nx = colour.shape
+    cap = int(max_links) if max_links is not None else 16 * (int(colour.max()) + 2)
+    links = np.zeros((max(cap, 1), 2), dtype=np.int32)
+    n = _load().orc_delaunay(nx, ny, int(bool(periodic_y)), colour.ctypes.data, cap, links.ctypes.data)
+    return links[:min(n, cap)].copy(), n
+
+
+def match(colour_past, periodic_y, centres_now):
+    """map[i] = past droplet in whose Voronoi cell the present centre i lies (reading R25)."""
+    colour_past = _i32(colour_past)
+    ny, nx = colour_past.shape
+    c = _c(centres_now).reshape(-1, 2)
+    m = np.zeros(len(c), dtype=np.int32)
+    _load().orc_match(nx, ny, int(bool(periodic_y)), colour_past.ctypes.data, _dp(c), len(c), m.ctypes.data)
+    return m
+
+
+def t1_events(links_past, links_now, map_now_to_past=None, max_events=4096):
+    """T1 events [e][4] = (a, b, c, d): link a-b replaced by link c-d (reading R25)."""
+    lp, ln = _i32(links_past).reshape(-1, 2), _i32(links_now).reshape(-1, 2)
+    mp = _i32(map_now_to_past) if map_now_to_past is not None else None
+    ev = np.zeros((max(max_events, 1), 4), dtype=np.int32)
+    n = _load().orc_t1_events(lp.ctypes.data, len(lp), ln.ctypes.data, len(ln), mp.ctypes.data if mp is not None else None,
+                              int(max_events), ev.ctypes.data)
+    return ev[:min(n, max_events)].copy(), n
 
 
 def lattice_weights():
