@@ -3,7 +3,7 @@
  *
  * The operation is the per-time-step update of TLBfind (arXiv 2109.12565); citations are
  * "PAPER L<line>" into /root/reference/PAPER.md plus the equation / section they fall in.
- * Readings R1..R22 of silent or garbled passages are listed in DESIGN.md.
+ * Readings R1..R26 of silent or garbled passages are listed in DESIGN.md.
  *
  * One step (tlb_step) computes, for every fluid site, from time-t populations only (R13):
  *   moments            rho_l = sum_i f_l,i ; T = sum_i g_i ; j = sum_l,i c_i f_l,i     Eqs. (4),(5),(17) L76-80, L165
@@ -224,6 +224,39 @@ int tlb_x_average_stress_host(tlb_handle* h, double* Pxy_av);
  * pointers (synchronises).  TLB_EINVAL on slab handles and for max_droplets > nx ny / 4. */
 int tlb_droplets(tlb_handle* h, double B_th, int32_t* labels, int32_t max_droplets, int32_t* n_droplets, double* stats);
 int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_droplets, int32_t* n_droplets, double* stats);
+
+/* Droplet analysis, second stage (section 2.4, Eq. (25)).  The paper describes it in prose and defers
+ * the details to its ref. [58]; readings R23-R26.  DEVICE pointers, asynchronous on the handle's stream,
+ * integer outputs bit-identical to the oracle's brute force.  The calls use the handle's scratch planes (they do not
+ * touch the populations); TLB_EINVAL on slab handles.
+ *
+ * tlb_voronoi (R23, "each point of the lattice is coloured by the label of the nearest centre of mass"):
+ *   centres [n][2] = { x, y } (e.g. columns 2, 3 of tlb_droplets' stats), colour [ny][nx] int32 = index k of the centre
+ *   with the smallest squared distance (x minimum image; y too with periodic_y), evaluated in fp64 without fused
+ *   multiply-add; ties go to the smallest index; -1 everywhere for n = 0.  n <= nx ny / 4.
+ * tlb_delaunay (R24, "The vertices at which adjacent digital Voronoi cells converge are used to identify the Delaunay
+ *   triangulation"): a vertex is a 2 x 2 block of sites (x periodic; y periodic with periodic_y, else the rows beyond
+ *   the flat walls carry a wall colour) holding >= 3 distinct colours; 3 colours link every pair of droplets in the
+ *   block, 4 colours the four side pairs and the main-diagonal pair (x, y)-(x+1, y+1).  links [max_links][2], a < b,
+ *   distinct, in lexicographic order; *n_links = their number (only the first max_links are written), or -1 if a
+ *   droplet has more than 32 links.  n = number of colours (droplets).
+ * tlb_droplet_match (R25): map[i] = colour_past at the site nearest to the present centre i (floor(c + 1/2), x wrapped,
+ *   y wrapped or clamped): the past droplet in whose Voronoi cell the present droplet lies.
+ * tlb_t1_events (R25, "the diagonal link between a and b is replaced by the link between c and d"): both link lists as
+ *   tlb_delaunay writes them; map (or NULL = identity; n_map entries) rewrites the ends of the present links into
+ *   indices of the past frame (links with an end mapped to < 0 or both ends on one droplet are dropped); n_droplets =
+ *   droplets of the past frame.  events [max_events][4] = { a, b, c, d }, a < b, c < d: a-b linked in the past and not
+ *   now, c-d now and not in the past, the sides a-c, a-d, b-c, b-d in both; lexicographic order; *n_events = their
+ *   number, or -1 on table overflow.
+ * tlb_droplet_nusselt (R26, Eq. (25)): nu[i] = [u_y^(H) T - kappa d_y T] / (kappa dT / ny) at the site nearest to centre
+ *   i, kappa and d_y T as in Eq. (24) / R10; 0 on a solid site.  TLB_ESTATE without a state. */
+int tlb_voronoi(tlb_handle* h, const double* centres, int32_t n, int32_t* colour);
+int tlb_delaunay(tlb_handle* h, const int32_t* colour, int32_t n, int32_t max_links, int32_t* n_links, int32_t* links);
+int tlb_droplet_match(tlb_handle* h, const int32_t* colour_past, const double* centres_now, int32_t n_now, int32_t* map);
+int tlb_t1_events(tlb_handle* h, const int32_t* links_past, int32_t n_past, const int32_t* links_now, int32_t n_now,
+                  const int32_t* map, int32_t n_map, int32_t n_droplets, int32_t max_events, int32_t* n_events,
+                  int32_t* events);
+int tlb_droplet_nusselt(tlb_handle* h, const double* centres, int32_t n, double* nu);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t tlb_launch_count(const tlb_handle* h);

@@ -619,6 +619,21 @@ void orc_voronoi(int nx, int ny, int periodic_y, const double *centres, int n, i
     }
 }
 
+/* the same for a list of m sites (site = y nx + x): lets a test check a large colouring on sampled sites */
+void orc_voronoi_at(int nx, int ny, int periodic_y, const double *centres, int n, const int64_t *sites, int m, int32_t *colour) {
+  for (int q = 0; q < m; q++) {
+    const int x = (int)(sites[q] % nx), y = (int)(sites[q] / nx);
+    int best = -1;
+    double bd = 0.0;
+    for (int k = 0; k < n; k++) {
+      const double dx = offset_to(x, centres[2 * k], nx, 1), dy = offset_to(y, centres[2 * k + 1], ny, periodic_y);
+      const double d2 = dx * dx + dy * dy;
+      if (best < 0 || d2 < bd) { best = k; bd = d2; }
+    }
+    colour[q] = best;
+  }
+}
+
 static int cmp_pair(const void *a, const void *b) {
   const int32_t *p = (const int32_t *)a, *q = (const int32_t *)b;
   if (p[0] != q[0]) return p[0] < q[0] ? -1 : 1;

@@ -61,6 +61,7 @@ def _load():
         lib.orc_droplets.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_void_p, ctypes.c_int, dp]
         i32p = ctypes.c_void_p
         lib.orc_voronoi.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_int, i32p]
+        lib.orc_voronoi_at.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_int, i32p, ctypes.c_int, i32p]
         lib.orc_delaunay.restype = ctypes.c_int
         lib.orc_delaunay.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, ctypes.c_int, i32p]
         lib.orc_match.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, dp, ctypes.c_int, i32p]
@@ -219,6 +220,15 @@ def voronoi(nx, ny, periodic_y, centres):
     colour = np.zeros((ny, nx), dtype=np.int32)
     _load().orc_voronoi(int(nx), int(ny), int(bool(periodic_y)), _dp(c), len(c), colour.ctypes.data)
     return colour
+
+
+def voronoi_at(nx, ny, periodic_y, centres, sites):
+    """Colours of the listed sites (y nx + x) only; the same brute force as voronoi()."""
+    c = _c(centres).reshape(-1, 2)
+    sites = np.ascontiguousarray(sites, dtype=np.int64)
+    out = np.zeros(len(sites), dtype=np.int32)
+    _load().orc_voronoi_at(int(nx), int(ny), int(bool(periodic_y)), _dp(c), len(c), sites.ctypes.data, len(sites), out.ctypes.data)
+    return out
 
 
 def delaunay(colour, periodic_y, max_links=None):

@@ -860,6 +860,67 @@ int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_d
   return check(h);
 }
 
+// ---- droplet analysis, second stage (section 2.4, Eq. (25); readings R23-R26).  Scratch planes fld[2], fld[3]
+// hold the cell grid / adjacency tables / events found; fld[3], fld[4] the fields of the Nusselt call.
+int tlb_voronoi(tlb_handle* h, const double* centres, int32_t n, int32_t* colour) {
+  if (!h || !colour || n < 0 || (n > 0 && !centres)) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
+  const size_t N = (size_t)h->d.nx * h->d.ny;
+  if ((size_t)n * 4 > N) return TLB_EINVAL;
+  TLB_ENTER(h);
+  h->launches += launch_voronoi(h->d, centres, n, reinterpret_cast<int*>(h->fld[2]), colour, h->st);
+  return check(h);
+}
+
+int tlb_delaunay(tlb_handle* h, const int32_t* colour, int32_t n, int32_t max_links, int32_t* n_links, int32_t* links) {
+  if (!h || !colour || !n_links || n < 0 || max_links < 0 || (max_links > 0 && !links)) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
+  const size_t N = (size_t)h->d.nx * h->d.ny;
+  if ((size_t)n * (kMaxDegree + 1) + 3 > 2 * N) return TLB_EINVAL;
+  TLB_ENTER(h);
+  h->launches += launch_delaunay(h->d, colour, n, reinterpret_cast<int*>(h->fld[2]), max_links, n_links, links, h->st);
+  return check(h);
+}
+
+int tlb_droplet_match(tlb_handle* h, const int32_t* colour_past, const double* centres_now, int32_t n_now, int32_t* map) {
+  if (!h || !colour_past || n_now < 0 || (n_now > 0 && (!centres_now || !map))) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
+  TLB_ENTER(h);
+  h->launches += launch_match(h->d, colour_past, centres_now, n_now, map, h->st);
+  return check(h);
+}
+
+int tlb_t1_events(tlb_handle* h, const int32_t* links_past, int32_t n_past, const int32_t* links_now, int32_t n_now,
+                  const int32_t* map, int32_t n_map, int32_t n_droplets, int32_t max_events, int32_t* n_events,
+                  int32_t* events) {
+  if (!h || !n_events || n_past < 0 || n_now < 0 || n_droplets < 0 || max_events < 0 || n_map < 0) return TLB_EINVAL;
+  if ((n_past > 0 && !links_past) || (n_now > 0 && !links_now) || (max_events > 0 && !events)) return TLB_EINVAL;
+  const size_t N = (size_t)h->d.nx * h->d.ny;
+  if (2 * (size_t)n_droplets * kMaxDegree > 2 * N || N < 8) return TLB_EINVAL;
+  TLB_ENTER(h);
+  // fld[2], fld[3] are adjacent planes: the two tables fill (part of) the first, the events found start at the second
+  int* scratch = reinterpret_cast<int*>(h->fld[2]);
+  size_t cap = (2 * N - 2) / 4;  // events that fit behind the two counters in fld[3]
+  if (cap > (size_t)1 << 20) cap = (size_t)1 << 20;
+  // launch_t1 lays the counters and the event list right behind the tables
+  h->launches += launch_t1(links_past, n_past, links_now, n_now, map, n_map, n_droplets, scratch, (int)cap, max_events,
+                           n_events, events, h->st);
+  return check(h);
+}
+
+int tlb_droplet_nusselt(tlb_handle* h, const double* centres, int32_t n, double* nu) {
+  if (!h || n < 0 || (n > 0 && (!centres || !nu))) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  FusedOut o{};
+  o.uy = h->fld[3]; o.T = h->fld[4];
+  int rc = fused_mode(h, 1, o);
+  if (rc != TLB_OK) return rc;
+  h->launches += launch_droplet_nusselt(h->d, h->fld[3], h->fld[4], centres, n, h->p.tau_g, nu, h->st);
+  return check(h);
+}
+
 int64_t tlb_launch_count(const tlb_handle* h) { return h ? h->launches : 0; }
 
 const char* tlb_error_string(int code) {

@@ -24,6 +24,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cmath>
+
 #include "../../include/tlb.h"
 
 namespace tlb {
@@ -125,6 +127,21 @@ int launch_label_merge(const Dev& d, int* labels, cudaStream_t st);
 int launch_label_flatten(const Dev& d, int* labels, cudaStream_t st);
 int launch_droplet_stats(const Dev& d, const int* labels, int* roots, int* sorted, unsigned long long* sums,
                          int max_droplets, int* n_out, double* stats, cudaStream_t st);
+// droplet analysis, second stage (tlb_analysis.cu)
+constexpr int kMaxDegree = 32;  // slots per droplet in the adjacency tables (a Delaunay vertex has 6 links on average)
+struct VorGrid {                // uniform grid of cells the centres are binned into
+  int gx, gy;
+  double inv_wx, inv_wy, wmin;  // 1 / cell width in x and y, the smaller width
+};
+VorGrid make_vor_grid(int nx, int ny, int n);
+int launch_voronoi(const Dev& d, const double* centres, int n, int* scratch, int* colour, cudaStream_t st);
+int launch_delaunay(const Dev& d, const int* colour, int n, int* scratch, int max_links, int* n_links, int* links,
+                    cudaStream_t st);
+int launch_match(const Dev& d, const int* colour_past, const double* centres_now, int n_now, int* map, cudaStream_t st);
+int launch_t1(const int* past, int n_past, const int* now, int n_now, const int* map, int n_map, int n, int* scratch, int cap,
+              int max_events, int* n_events, int* events, cudaStream_t st);
+int launch_droplet_nusselt(const Dev& d, const double* uy, const double* T, const double* centres, int n, double tau_g,
+                           double* nu, cudaStream_t st);
 int configure_kernels();  // opt in to the dynamic shared memory the fused kernel needs; 0 on success
 int default_seg_rows(int nx, int ny);
 

@@ -283,3 +283,12 @@ def test_droplet_nusselt_reads_the_nearest_site(oracle_mod):
         dyT = 0.5 * (T[y + 1, x] + T[y, x]) - 0.5 * (T[y, x] + T[y - 1, x])
         exp.append((uy[y, x] * T[y, x] - kappa * dyT) / (kappa * 1.0 / ny))
     assert np.allclose(o.droplet_nusselt(centres), exp, rtol=1e-12, atol=1e-15)
+
+
+def test_voronoi_at_is_voronoi_on_listed_sites(oracle_mod):
+    rng = np.random.default_rng(4)
+    nx, ny = 50, 31
+    c = rng.random((9, 2)) * [nx, ny]
+    full = oracle_mod.voronoi(nx, ny, 0, c)
+    sites = rng.integers(0, nx * ny, 200)
+    assert (oracle_mod.voronoi_at(nx, ny, 0, c, sites) == full.ravel()[sites]).all()
