@@ -239,6 +239,31 @@ def run_ours(args, rank, world):
                     "sites_min": float(st[:min(k, cap), 1].min()) if k else None,
                     "sites_max": float(st[:min(k, cap), 1].max()) if k else None,
                     "call": "tlb_droplets (fields pass for rho_A, threshold, union-find labelling, flatten, statistics)"}
+        # second stage (R23-R26): digital Voronoi colouring of the centres, Delaunay links, droplet Nusselt numbers
+        kk = min(k, cap)
+        if kk > 0:
+            cen = st[:kk, 2:4].contiguous()
+            col = torch.empty((ny, nx), dtype=torch.int32, device=dev)
+            nl = torch.zeros(1, dtype=torch.int32, device=dev)
+            lk = torch.zeros((16 * kk, 2), dtype=torch.int32, device=dev)
+            nu = torch.zeros(kk, dtype=torch.float64, device=dev)
+
+            def stage2():
+                assert t.lib.tlb_voronoi(t.h, cen.data_ptr(), kk, col.data_ptr()) == 0
+                assert t.lib.tlb_delaunay(t.h, col.data_ptr(), kk, 16 * kk, nl.data_ptr(), lk.data_ptr()) == 0
+                assert t.lib.tlb_droplet_nusselt(t.h, cen.data_ptr(), kk, nu.data_ptr()) == 0
+            stage2()
+            torch.cuda.synchronize()
+            d0.record(t.stream)
+            for _ in range(20):
+                stage2()
+            d1.record(t.stream)
+            torch.cuda.synchronize()
+            s2 = d0.elapsed_time(d1) / 20
+            droplets.update({"stage2_ms": s2, "stage2_lb_steps": s2 / step_ms, "n_links": int(nl.item()),
+                             "whole_analysis_lb_steps": (dms + s2) / step_ms,
+                             "stage2_call": "tlb_voronoi + tlb_delaunay + tlb_droplet_nusselt on the centres of tlb_droplets"})
+            del cen, col, nl, lk, nu
         del lab, nd, st
 
     # ---- optional long run with the observables logged (BASELINE config 2: Nu and mass every 1000 steps)
