@@ -10,7 +10,7 @@
  *
  * The method is an explicit iteration, so the oracle follows it step by step in the
  * paper's order and notation (PAPER Eqs. (1)-(22)); readings of silent / garbled passages
- * are the ones listed in DESIGN.md ("Readings R1..R26").  No blocking, fusion or reordering:
+ * are the ones listed in DESIGN.md ("Readings R1..R29").  No blocking, fusion or reordering:
  * every sub-step is a full sweep over the lattice writing a full array.
  *
  * Parity pins (tests/test_oracle_pins.py, all run with -m "not gpu"):
@@ -37,6 +37,9 @@
  *                      wall mirror images) of jittered triangular arrangements; a hand-made diagonal flip and
  *                      flips of a triangulated grid; Nu_drop = 1 + U T(y_i) ny / (kappa dT) in a uniform stream
  *                      (tests/test_oracle_analysis.py)               section 2.4, Eq. (25) (R23-R26)
+ *   rough walls        alpha = 0 is the rectangular post mask; site counts of the trapezoid; vertical side of the
+ *                      asymmetric one; mirror images                          section 4, Table A.6 (R27)
+ *   perturbation       densities unchanged, momentum rho du, u^(H) = du on a rest state         L322 (R29)
  *   posts / corners    second, independently written streaming formulation
  *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
  *                      pull of orc_step; beyond that and mass conservation the post-corner
@@ -768,6 +771,52 @@ void orc_droplet_nusselt(orc_state *s, const double *centres, int n, double *nu)
     else dn = 0.5 * (s->T[k] + s->T[IDX(s, x, s->p.periodic_y ? wrap(y - 1, ny) : y - 1)]);
     nu[i] = (s->uHy[k] * s->T[k] - kappa * (up - dn)) / (kappa * DT / ny);
   }
+}
+
+/* ---- Workflow pieces of the paper (readings R27, R29 of DESIGN.md) ---- */
+
+/* R27, rough walls with trapezoidal obstacles (section 4, Fig. 7(a) -- the figure is missing --, Table A.6:
+ * roughWallUp, roughWallDown, width, height, lambda, alpha, asymmetric): "The height, the width, the periodicity
+ * (via lambda), and the angle (via alpha) can be varied"; alpha = 0 gives "a simple rectangular-shape roughness".
+ * Reading: an obstacle stands on the wall every `lambda` nodes; in the row j = 0 .. height - 1 counted from the wall
+ * it covers the nodes l(j) <= (x mod lambda) < width - r(j), r(j) = floor(j tan(alpha)) (alpha in radians), l(j) =
+ * r(j) for a symmetric trapezoid and 0 (a vertical side) for the asymmetric one.  The top wall carries the mirror
+ * image in y.  solid[ny][nx] is overwritten. */
+void orc_rough_walls(int nx, int ny, int up, int down, int width, int height, int lambda, double alpha, int asymmetric,
+                     uint8_t *solid) {
+  const double t = tan(alpha);
+  memset(solid, 0, (size_t)nx * ny);
+  for (int j = 0; j < height && j < ny; j++) {
+    const int r = (int)floor((double)j * t), l = asymmetric ? 0 : r;
+    for (int x = 0; x < nx; x++) {
+      const int m = x % lambda;
+      if (m < l || m >= width - r) continue;
+      if (down) solid[(size_t)j * nx + x] = 1;
+      if (up) solid[(size_t)(ny - 1 - j) * nx + x] = 1;
+    }
+  }
+}
+
+/* R29, initial velocity perturbation (L322: "a finite perturbation is necessary to destabilise the conductive
+ * state"; "initial velocity perturbation" 1e-4 in Table A.5; its shape is not given).  Reading: one convection
+ * roll pair, du = (0, A sin(2 pi x / nx) sin(pi (y + 1/2) / ny)), given to both fluids by shifting every population of
+ * a fluid site by the first-order equilibrium term, f_l,i += 3 w_i rho_l (c_i . du) with rho_l = sum_i f_l,i: each
+ * component's density is unchanged (sum_i w_i c_i = 0) and its momentum grows by rho_l du (sum_i w_i c_i c_i = 1/3). */
+void orc_perturb_velocity(orc_state *s, double amplitude) {
+  const int nx = s->nx, ny = s->ny;
+  const double pi = 3.14159265358979323846;
+  for (int y = 0; y < ny; y++)
+    for (int x = 0; x < nx; x++) {
+      if (s->solid[IDX(s, x, y)]) continue;
+      const double duy = amplitude * sin(2.0 * pi * (double)x / (double)nx) * sin(pi * ((double)y + 0.5) / (double)ny);
+      double ra = 0.0, rb = 0.0;
+      for (int i = 0; i < 9; i++) { ra += s->fA[PIDX(s, i, x, y)]; rb += s->fB[PIDX(s, i, x, y)]; }
+      for (int i = 0; i < 9; i++) {
+        const double cu = (double)CY[i] * duy;
+        s->fA[PIDX(s, i, x, y)] += 3.0 * W[i] * ra * cu;
+        s->fB[PIDX(s, i, x, y)] += 3.0 * W[i] * rb * cu;
+      }
+    }
 }
 
 /* lattice constants exported for the weight-invariant pins */

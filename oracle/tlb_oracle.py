@@ -68,6 +68,8 @@ def _load():
         lib.orc_t1_events.restype = ctypes.c_int
         lib.orc_t1_events.argtypes = [i32p, ctypes.c_int, i32p, ctypes.c_int, i32p, ctypes.c_int, i32p]
         lib.orc_droplet_nusselt.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp]
+        lib.orc_rough_walls.argtypes = [ctypes.c_int] * 7 + [ctypes.c_double, ctypes.c_int, ctypes.c_void_p]
+        lib.orc_perturb_velocity.argtypes = [ctypes.c_void_p, ctypes.c_double]
         lib.orc_w.restype = ctypes.c_double
         lib.orc_w.argtypes = [ctypes.c_int, ctypes.c_int]
         lib.orc_p.restype = ctypes.c_double
@@ -208,6 +210,22 @@ def _droplet_nusselt(self, centres):
 
 
 Oracle.droplet_nusselt = _droplet_nusselt
+
+
+def _perturb_velocity(self, amplitude):
+    """One roll pair of amplitude A added to both fluids' momentum (reading R29)."""
+    self.lib.orc_perturb_velocity(self.h, float(amplitude))
+
+
+Oracle.perturb_velocity = _perturb_velocity
+
+
+def rough_walls(nx, ny, up, down, width, height, lam, alpha, asymmetric):
+    """Obstacle mask [ny][nx] uint8 of trapezoidal rough walls (reading R27)."""
+    solid = np.zeros((ny, nx), dtype=np.uint8)
+    _load().orc_rough_walls(int(nx), int(ny), int(up), int(down), int(width), int(height), int(lam), float(alpha),
+                            int(asymmetric), solid.ctypes.data)
+    return solid
 
 
 def _i32(a):

@@ -110,13 +110,27 @@ def place_droplets(nx, ny, seed, n_droplets, radius, min_gap, post_h=0):
     return centres
 
 
+def honeycomb_centres(nx, ny, ndx, ndy, post_h=0):
+    """ndx x ndy centres in a honeycomb (triangular) arrangement between the walls / posts, the paper's own
+    initialisation ("droplet initialisation = 1"): row j at y = post_h + (j + 1/2) (ny - 2 post_h) / ndy,
+    column i at x = (i + 1/4 + (j mod 2) / 2) nx / ndx."""
+    j, i = np.divmod(np.arange(ndx * ndy), ndx)
+    ax = float(nx) / float(ndx)
+    ay = (float(ny) - 2.0 * float(post_h)) / float(ndy)
+    cx = (i.astype(np.float64) + 0.25 + 0.5 * (j % 2).astype(np.float64)) * ax
+    cy = float(post_h) + (j.astype(np.float64) + 0.5) * ay
+    return np.stack([cx, cy], 1)
+
+
 def initial_fields(nx, ny, seed, n_droplets, droplet_radius, min_gap, rho_in, rho_out, noise_amp,
-                   T_bottom, T_top, solid=None, post_h=0):
+                   T_bottom, T_top, solid=None, post_h=0, centres=None):
     """(rho_A, rho_B, T) of the input recipe: droplets rich in A, matrix rich in B, seeded uniform
-    noise on fluid sites, linear temperature profile between the walls."""
+    noise on fluid sites, linear temperature profile between the walls.  `centres` (n, 2)
+    replaces the random sequential addition (e.g. honeycomb_centres)."""
     inside = np.zeros((ny, nx), dtype=bool)
-    if n_droplets > 0:
-        centres = place_droplets(nx, ny, seed, n_droplets, droplet_radius, min_gap, post_h)
+    if centres is not None or n_droplets > 0:
+        if centres is None:
+            centres = place_droplets(nx, ny, seed, n_droplets, droplet_radius, min_gap, post_h)
         r2 = float(droplet_radius) * float(droplet_radius)
         rr = int(np.ceil(droplet_radius)) + 1
         for cx, cy in centres:

@@ -292,3 +292,74 @@ def test_voronoi_at_is_voronoi_on_listed_sites(oracle_mod):
     full = oracle_mod.voronoi(nx, ny, 0, c)
     sites = rng.integers(0, nx * ny, 200)
     assert (oracle_mod.voronoi_at(nx, ny, 0, c, sites) == full.ravel()[sites]).all()
+
+
+# ---------------------------------------------------------------- R27: trapezoidal rough walls; R29: perturbation
+
+def test_rough_walls_rectangles_are_the_post_mask(oracle_mod):
+    """alpha = 0: "a simple rectangular-shape roughness" (L366) = the structured posts of the headline config."""
+    from paper_2109_12565_b200 import inputs
+    for nx, ny, w, h, lam in ((64, 24, 4, 4, 16), (150, 40, 10, 7, 30), (33, 12, 5, 3, 11)):
+        assert (oracle_mod.rough_walls(nx, ny, 1, 1, w, h, lam, 0.0, 0) == inputs.post_mask(nx, ny, w, h, lam)).all()
+        only_down = oracle_mod.rough_walls(nx, ny, 0, 1, w, h, lam, 0.0, 1)
+        assert only_down[ny // 2:].sum() == 0 and (only_down[:h] == inputs.post_mask(nx, ny, w, h, lam)[:h]).all()
+
+
+@pytest.mark.parametrize("asym", [0, 1])
+def test_rough_walls_trapezoid_shape(oracle_mod, asym):
+    """Table A.6's obstacle: width 10, lambda 150, alpha 0.25 (L446-451).  Row j from the wall loses floor(j tan alpha)
+    nodes on the inclined side(s): site counts, the vertical side of the asymmetric shape, the mirror symmetry of the
+    symmetric one, the top wall as the y-mirror of the bottom wall."""
+    nx, ny, w, h, lam, alpha = 300, 60, 10, 9, 150, 0.25
+    m = oracle_mod.rough_walls(nx, ny, 1, 1, w, h, lam, alpha, asym)
+    cut = [int(np.floor(j * np.tan(alpha))) for j in range(h)]
+    assert cut == [0, 0, 0, 0, 1, 1, 1, 1, 2]
+    for j in range(h):
+        expect = w - cut[j] * (1 if asym else 2)
+        assert m[j].sum() == expect * (nx // lam)
+        assert (m[j] == m[ny - 1 - j]).all()
+        row = m[j, :lam]
+        first, last = np.nonzero(row)[0][[0, -1]]
+        assert first == (0 if asym else cut[j]) and last == w - 1 - cut[j]
+        assert row[first:last + 1].all()                                   # one solid run per obstacle
+    assert m[h:ny - h].sum() == 0
+    assert (m[:, :lam] == m[:, lam:2 * lam]).all()                         # period lambda
+
+
+def test_velocity_perturbation_closed_form(oracle_mod):
+    """R29: densities unchanged, each fluid's momentum grows by rho_l du, so on a rest state without forces
+    u^(H) = du = (0, A sin(2 pi x / nx) sin(pi (y + 1/2) / ny)); solid sites untouched; A = 0 is a no-op."""
+    nx, ny, A = 24, 16, 1e-3
+    rng = np.random.default_rng(0)
+    rA, rB = 0.5 + rng.random((ny, nx)), 0.2 + rng.random((ny, nx))
+    solid = np.zeros((ny, nx), np.uint8)
+    solid[:2, 3:6] = 1
+    o = oracle_mod.Oracle(nx, ny, tau=1.0, thermal=0)
+    o.set_solid(solid)
+    o.set_fields(rA, rB, np.zeros((ny, nx)))
+    f0 = [p.copy() for p in o.get_populations()]
+    o.perturb_velocity(0.0)
+    assert all((p == q).all() for p, q in zip(o.get_populations(), f0))
+    o.perturb_velocity(A)
+    fA, fB, g = o.get_populations()
+    fl = solid == 0
+    assert (g == f0[2]).all() and (fA[:, ~fl] == f0[0][:, ~fl]).all()
+    assert np.abs(fA.sum(0) - f0[0].sum(0)).max() < 2e-16 * 4 and np.abs(fB.sum(0) - f0[1].sum(0)).max() < 2e-16 * 4
+    du = A * np.sin(2 * np.pi * np.arange(nx) / nx)[None, :] * np.sin(np.pi * (np.arange(ny) + 0.5) / ny)[:, None]
+    jyA, jxA = (fA * _CY).sum(0), (fA * _CX).sum(0)
+    assert np.abs(jyA - f0[0].sum(0) * du)[fl].max() < 2e-16 and np.abs(jxA)[fl].max() < 2e-16   # rounding of sums of 9 terms ~ 0.1
+    rho_A, rho_B, u, T = o.fields()
+    assert np.abs(u[1] - du)[fl].max() < 3e-16 and np.abs(u[0])[fl].max() < 3e-16 and np.abs(du).max() > 0.9 * A
+
+
+def test_honeycomb_centres_arrangement():
+    """L266: honeycomb structure of ndx x ndy droplets: equal spacing along x, rows offset by half a spacing."""
+    from paper_2109_12565_b200 import inputs
+    nx, ny, ndx, ndy = 120, 104, 6, 6
+    c = inputs.honeycomb_centres(nx, ny, ndx, ndy)
+    assert c.shape == (36, 2)
+    rows = c.reshape(ndy, ndx, 2)
+    assert np.allclose(np.diff(rows[:, :, 0], axis=1), nx / ndx) and np.allclose(rows[1, :, 0] - rows[0, :, 0], nx / ndx / 2)
+    assert np.allclose(np.diff(rows[:, 0, 1]), ny / ndy) and rows[0, 0, 1] == ny / ndy / 2
+    cp = inputs.honeycomb_centres(nx, ny, ndx, ndy, post_h=4)
+    assert cp[:, 1].min() == 4 + (ny - 8) / ndy / 2 and np.isclose(cp[:, 1].max(), ny - 4 - (ny - 8) / ndy / 2)
