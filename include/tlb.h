@@ -74,7 +74,8 @@ enum {
   TLB_EINVAL = -1,     /* bad size / parameter / NULL pointer / workspace too small              */
   TLB_ESTATE = -2,     /* step / fields / observables before any state was set                   */
   TLB_ECUDA = -3,      /* a CUDA call failed (sticky on the handle); see tlb_last_cuda_error      */
-  TLB_EPLACEMENT = -4  /* tlb_init could not place n_droplets within 1000 * n_droplets candidates */
+  TLB_EPLACEMENT = -4, /* tlb_init could not place n_droplets within 1000 * n_droplets candidates */
+  TLB_EIO = -5         /* a checkpoint file could not be opened, or has the wrong size              */
 };
 
 /* POD, passed by pointer, copied by tlb_create. */
@@ -136,6 +137,40 @@ int tlb_seg_rows(const tlb_handle* h);
  * discs by random sequential addition, +noise, linear T profile (L314), populations at rest
  * equilibrium f = w rho, g = w T (R14).  Bit-identical to paper_2109_12565_b200/inputs.py. */
 int tlb_init(tlb_handle* h, uint64_t seed);
+
+/* The same with the paper's own droplet arrangement ("droplet initialisation = 1", L266: "we initialise the soft domains
+ * in an honeycomb structure, where we establish the total number of droplets by calibrating the relative number of
+ * droplets along x and y"): ndx x ndy discs of params.droplet_radius, row j at y = post_h + (j + 1/2)(ny - 2 post_h)/ndy,
+ * column i at x = (i + 1/4 + (j mod 2)/2) nx/ndx.  Bit-identical to inputs.honeycomb_centres + inputs.initial_fields.
+ * TLB_EINVAL for ndx, ndy < 1 or 2 ndx ndy > nx ny. */
+int tlb_init_honeycomb(tlb_handle* h, int32_t ndx, int32_t ndy, uint64_t seed);
+
+/* Rough walls with trapezoidal obstacles (section 4, Fig. 7(a), Table A.6; reading R27): replaces the obstacle
+ * mask like tlb_set_solid (state and graphs are dropped).  An obstacle stands on the wall every `lambda` nodes; in row
+ * j = 0 .. height - 1 counted from the wall it covers l(j) <= (x mod lambda) < width - r(j), r(j) = floor(j tan(alpha))
+ * (alpha in radians, evaluated on the host), l(j) = r(j), or 0 when `asymmetric`; the top wall carries the y-mirror
+ * image.  alpha = 0 gives the rectangular posts of tlb_params.  TLB_EINVAL with periodic_y, lambda < 1,
+ * width > lambda, width or height < 0, obstacles of the two walls touching (2 height > ny). */
+typedef struct tlb_rough_walls {
+  double alpha;                         /* inclination of the trapezoid's side(s), radians; Table A.6: 0.25  */
+  int32_t up, down;                     /* roughWallUp, roughWallDown                                          */
+  int32_t width, height, lambda;        /* base width, height, period (nodes)                                  */
+  int32_t asymmetric;                   /* 1: only the right-hand side is inclined                             */
+} tlb_rough_walls;
+int tlb_set_rough_walls(tlb_handle* h, const tlb_rough_walls* r);
+
+/* Initial velocity perturbation (L322 "a finite perturbation is necessary to destabilise the conductive state",
+ * Table A.5; reading R29): adds the roll pair du = (0, A sin(2 pi x/nx) sin(pi (y + 1/2)/ny)) to both fluids of the
+ * current state, f_l,i += 3 w_i rho_l (c_i . du) on fluid sites (densities unchanged, momentum + rho_l du).  TLB_ESTATE
+ * without a state. */
+int tlb_perturb_velocity(tlb_handle* h, double amplitude);
+
+/* Checkpoint files (Table C.11: "conf1_#.in / conf2_#.in / confG_#.in ... populations field dumped as a binary
+ * file"; restart L324): <dir>/conf1_<index>.in, conf2_<index>.in, confG_<index>.in, each the raw little-endian fp64 array
+ * [9][ny][nx] of tlb_get_populations (direction order R1; 0 on solid sites).  _read restores such a dump into a handle
+ * of the same nx, ny (the obstacle mask is not part of a dump: set it first).  Synchronise; TLB_EIO on a file error. */
+int tlb_write_checkpoint(tlb_handle* h, const char* dir, int32_t index);
+int tlb_read_checkpoint(tlb_handle* h, const char* dir, int32_t index);
 
 /* Arbitrary obstacle mask [ny][nx], non-zero = solid (flag field, L286).  Resets the state. */
 int tlb_set_solid(tlb_handle* h, const uint8_t* solid);

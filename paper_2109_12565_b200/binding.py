@@ -16,11 +16,12 @@ SOURCES = ["tlb_step.cu", "tlb_aux.cu", "tlb_analysis.cu", "tlb_api.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
-TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT = 0, -1, -2, -3, -4
+TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT, TLB_EIO = 0, -1, -2, -3, -4, -5
 
 # every symbol include/tlb.h declares
 SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_slab_workspace_bytes",
-           "tlb_create_slab", "tlb_slab_layout", "tlb_halo_bytes", "tlb_seg_rows", "tlb_init", "tlb_set_solid",
+           "tlb_create_slab", "tlb_slab_layout", "tlb_halo_bytes", "tlb_seg_rows", "tlb_init", "tlb_init_honeycomb",
+           "tlb_set_rough_walls", "tlb_perturb_velocity", "tlb_write_checkpoint", "tlb_read_checkpoint", "tlb_set_solid",
            "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
            "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step",
            "tlb_slab_step_edges", "tlb_slab_step_interior", "tlb_slab_step_finish", "tlb_halo_pack", "tlb_halo_unpack",
@@ -38,6 +39,11 @@ class TLBParams(ctypes.Structure):
         "T_bottom", "T_top", "T_ref", "alpha_g", "body_ax", "u_wall_bottom", "u_wall_top",
         "droplet_radius", "min_gap", "rho_in", "rho_out", "noise_amp")] + [(n, ctypes.c_int32) for n in (
             "n_droplets", "periodic_y", "thermal", "post_w", "post_h", "post_period", "pop_precision", "reserved")]
+
+
+class TLBRoughWalls(ctypes.Structure):
+    """Mirror of `struct tlb_rough_walls` (include/tlb.h)."""
+    _fields_ = [("alpha", ctypes.c_double)] + [(n, ctypes.c_int32) for n in ("up", "down", "width", "height", "lam", "asymmetric")]
 
 
 class TLBError(RuntimeError):
@@ -86,6 +92,11 @@ def load_library():
     lib.tlb_create.argtypes = [i32, i32, pp, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
     lib.tlb_destroy.argtypes = [vp]
     lib.tlb_init.argtypes = [vp, ctypes.c_uint64]
+    lib.tlb_init_honeycomb.argtypes = [vp, i32, i32, ctypes.c_uint64]
+    lib.tlb_set_rough_walls.argtypes = [vp, ctypes.POINTER(TLBRoughWalls)]
+    lib.tlb_perturb_velocity.argtypes = [vp, ctypes.c_double]
+    lib.tlb_write_checkpoint.argtypes = [vp, ctypes.c_char_p, i32]
+    lib.tlb_read_checkpoint.argtypes = [vp, ctypes.c_char_p, i32]
     lib.tlb_set_solid.argtypes = [vp, dp]
     lib.tlb_set_solid_host.argtypes = [vp, dp]
     for name in ("tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations", "tlb_get_populations",
@@ -264,6 +275,23 @@ class TLB:
         a, b, c = (self._host(v, (9, self.ny, self.nx)) for v in out)
         self._chk(self.lib.tlb_get_populations_host(self.h, a.data_ptr(), b.data_ptr(), c.data_ptr()))
         return [a, b, c]
+
+    def init_honeycomb(self, ndx, ndy, seed):
+        self._chk(self.lib.tlb_init_honeycomb(self.h, int(ndx), int(ndy), int(seed)))
+
+    def set_rough_walls(self, up, down, width, height, lam, alpha, asymmetric):
+        r = TLBRoughWalls(alpha=float(alpha), up=int(up), down=int(down), width=int(width), height=int(height),
+                          lam=int(lam), asymmetric=int(asymmetric))
+        self._chk(self.lib.tlb_set_rough_walls(self.h, ctypes.byref(r)))
+
+    def perturb_velocity(self, amplitude):
+        self._chk(self.lib.tlb_perturb_velocity(self.h, float(amplitude)))
+
+    def write_checkpoint(self, directory, index=0):
+        self._chk(self.lib.tlb_write_checkpoint(self.h, os.fsencode(directory), int(index)))
+
+    def read_checkpoint(self, directory, index=0):
+        self._chk(self.lib.tlb_read_checkpoint(self.h, os.fsencode(directory), int(index)))
 
     def step(self, n=1):
         self._chk(self.lib.tlb_step(self.h, int(n)))

@@ -1,8 +1,10 @@
 // tlb_api.cu -- the C ABI of include/tlb.h: handle, parameter checks, workspace carving, and the
 // host side of every call (argument marshalling and kernel launches only; no lattice arithmetic).
 #include <cmath>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <string>
 #include <new>
 #include <vector>
 
@@ -470,23 +472,62 @@ int tlb_halo_bytes(const tlb_handle* h, size_t* bytes) {
 
 int tlb_seg_rows(const tlb_handle* h) { return h ? h->seg_rows : TLB_EINVAL; }
 
+// seeded initial state from a list of disc centres (host): posts from params, discs, noise, linear T (input recipe)
+static int init_from_centres(tlb_handle* h, uint64_t seed, const std::vector<double>& c, double* dev_centres) {
+  const int n = (int)(c.size() / 2);
+  if (n > 0) {
+    cu(h, cudaMemcpyAsync(dev_centres, c.data(), c.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
+    cu(h, cudaStreamSynchronize(h->st));  // `c` is pageable and dies with the caller's frame
+  }
+  uint8_t* inside = reinterpret_cast<uint8_t*>(h->fld[2]);
+  cu(h, cudaMemsetAsync(inside, 0, (size_t)h->d.nx * h->d.ny, h->st));
+  h->launches += launch_init(h->d, h->p, seed, dev_centres, n, inside, h->solid, h->fld[0], h->fld[1], h->fld[4], h->st);
+  int rc = rebuild_links(h);
+  if (rc != TLB_OK) return rc;
+  h->launches += launch_set_fields(h->d, h->fld[0], h->fld[1], h->fld[4], h->S[h->cur], h->st);
+  return after_state_set(h);
+}
+
 int tlb_init(tlb_handle* h, uint64_t seed) {
   if (!h) return TLB_EINVAL;
   TLB_ENTER(h);
   std::vector<double> c;
   if (!place_droplets(h->d.nx, h->d.ny_glob, seed, h->p, c)) return TLB_EPLACEMENT;
-  const int n = (int)(c.size() / 2);
-  if (n > 0) {
-    cu(h, cudaMemcpyAsync(h->centres, c.data(), c.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
-    cu(h, cudaStreamSynchronize(h->st));  // `c` is pageable and dies with this frame
-  }
-  uint8_t* inside = reinterpret_cast<uint8_t*>(h->fld[2]);
-  cu(h, cudaMemsetAsync(inside, 0, (size_t)h->d.nx * h->d.ny, h->st));
-  h->launches += launch_init(h->d, h->p, seed, h->centres, n, inside, h->solid, h->fld[0], h->fld[1], h->fld[4], h->st);
-  int rc = rebuild_links(h);
-  if (rc != TLB_OK) return rc;
-  h->launches += launch_set_fields(h->d, h->fld[0], h->fld[1], h->fld[4], h->S[h->cur], h->st);
-  return after_state_set(h);
+  return init_from_centres(h, seed, c, h->centres);
+}
+
+int tlb_init_honeycomb(tlb_handle* h, int32_t ndx, int32_t ndy, uint64_t seed) {
+  if (!h || ndx < 1 || ndy < 1) return TLB_EINVAL;
+  const size_t N = (size_t)h->d.nx * h->d.ny;
+  if (2 * (size_t)ndx * (size_t)ndy > N) return TLB_EINVAL;  // the centres are staged in a scratch plane
+  TLB_ENTER(h);
+  // inputs.honeycomb_centres, operation for operation (this file is compiled without FMA contraction)
+  const double ax = (double)h->d.nx / (double)ndx;
+  const double ay = ((double)h->d.ny_glob - 2.0 * (double)h->p.post_h) / (double)ndy;
+  std::vector<double> c;
+  c.reserve(2 * (size_t)ndx * ndy);
+  for (int j = 0; j < ndy; j++)
+    for (int i = 0; i < ndx; i++) {
+      c.push_back(((double)i + 0.25 + 0.5 * (double)(j % 2)) * ax);
+      c.push_back((double)h->p.post_h + ((double)j + 0.5) * ay);
+    }
+  return init_from_centres(h, seed, c, h->fld[3]);
+}
+
+int tlb_set_rough_walls(tlb_handle* h, const tlb_rough_walls* r) {
+  if (!h || !r) return TLB_EINVAL;
+  if (h->p.periodic_y || r->lambda < 1 || r->width < 0 || r->width > r->lambda || r->height < 0) return TLB_EINVAL;
+  if ((r->up && r->down ? 2 * (long long)r->height : (long long)r->height) > h->d.ny_glob) return TLB_EINVAL;
+  TLB_ENTER(h);
+  std::vector<int> cut((size_t)(r->height > 0 ? r->height : 1), 0);
+  const double t = std::tan(r->alpha);
+  for (int j = 0; j < r->height; j++) cut[(size_t)j] = (int)std::floor((double)j * t);
+  int* dcut = reinterpret_cast<int*>(h->fld[2]);  // height <= ny ints
+  cu(h, cudaMemcpyAsync(dcut, cut.data(), cut.size() * sizeof(int), cudaMemcpyHostToDevice, h->st));
+  cu(h, cudaStreamSynchronize(h->st));
+  h->launches += launch_rough_walls(h->d, dcut, r->height, r->up ? 1 : 0, r->down ? 1 : 0, r->width, r->lambda,
+                                    r->asymmetric ? 1 : 0, h->solid, h->st);
+  return rebuild_links(h);
 }
 
 int tlb_set_solid(tlb_handle* h, const uint8_t* solid) {
@@ -569,6 +610,58 @@ int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g) {
   if (!h->d.thermal && !h->stage) h->launches += launch_copy_g(h->d, h->S[h->cur], h->S[1 - h->cur], h->st);
   cu(h, cudaStreamSynchronize(h->st));
   return check(h);
+}
+
+int tlb_perturb_velocity(tlb_handle* h, double amplitude) {
+  if (!h) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  TLB_ENTER(h);
+  // time-t populations into the staging area, perturbed there, and back (the route of the *_host population calls)
+  const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
+  double* stage = h->stage ? h->stage : static_cast<double*>(h->S[1 - h->cur]);
+  h->launches += launch_gather(h->d, h->S[h->cur], stage, stage + n9, stage + 2 * n9, h->st);
+  h->launches += launch_perturb(h->d, amplitude, stage, stage + n9, h->st);
+  h->launches += launch_scatter(h->d, stage, stage + n9, stage + 2 * n9, h->S[h->cur], h->st);
+  return after_state_set(h);
+}
+
+static std::string checkpoint_name(const char* dir, const char* stem, int index) {
+  return std::string(dir) + "/" + stem + "_" + std::to_string(index) + ".in";
+}
+
+int tlb_write_checkpoint(tlb_handle* h, const char* dir, int32_t index) {
+  if (!h || !dir) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
+  std::vector<double> buf;
+  try { buf.resize(3 * n9); } catch (...) { return TLB_EINVAL; }
+  int rc = tlb_get_populations_host(h, buf.data(), buf.data() + n9, buf.data() + 2 * n9);
+  if (rc != TLB_OK) return rc;
+  const char* stems[3] = {"conf1", "conf2", "confG"};
+  for (int k = 0; k < 3; k++) {
+    FILE* f = std::fopen(checkpoint_name(dir, stems[k], index).c_str(), "wb");
+    if (!f) return TLB_EIO;
+    const size_t w = std::fwrite(buf.data() + k * n9, sizeof(double), n9, f);
+    if (std::fclose(f) != 0 || w != n9) return TLB_EIO;
+  }
+  return TLB_OK;
+}
+
+int tlb_read_checkpoint(tlb_handle* h, const char* dir, int32_t index) {
+  if (!h || !dir) return TLB_EINVAL;
+  const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
+  std::vector<double> buf;
+  try { buf.resize(3 * n9); } catch (...) { return TLB_EINVAL; }
+  const char* stems[3] = {"conf1", "conf2", "confG"};
+  for (int k = 0; k < 3; k++) {
+    FILE* f = std::fopen(checkpoint_name(dir, stems[k], index).c_str(), "rb");
+    if (!f) return TLB_EIO;
+    const size_t r = std::fread(buf.data() + k * n9, sizeof(double), n9, f);
+    const bool more = std::fgetc(f) != EOF;  // a dump of another lattice size
+    std::fclose(f);
+    if (r != n9 || more) return TLB_EIO;
+  }
+  return tlb_set_populations_host(h, buf.data(), buf.data() + n9, buf.data() + 2 * n9);
 }
 
 int tlb_step(tlb_handle* h, int64_t n) {
@@ -930,6 +1023,7 @@ const char* tlb_error_string(int code) {
     case TLB_ESTATE: return "no state (call tlb_init, tlb_set_fields or tlb_set_populations first) or slab step calls out of order";
     case TLB_ECUDA: return "CUDA error (see tlb_last_cuda_error); there is no CPU fallback";
     case TLB_EPLACEMENT: return "tlb_init could not place n_droplets by random sequential addition";
+    case TLB_EIO: return "checkpoint file missing, unreadable, unwritable or of another lattice size";
   }
   return "unknown error code";
 }

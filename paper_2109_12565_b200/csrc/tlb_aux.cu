@@ -221,6 +221,39 @@ x_average_kernel(const Dev d, const double* __restrict__ ux, double* __restrict_
   }
 }
 
+// ---- trapezoidal rough walls (reading R27): cut[j] = floor(j tan(alpha)) for the rows j = 0 .. height - 1 from the wall
+__global__ void rough_walls_kernel(const Dev d, const int* __restrict__ cut, int height, int up, int down, int width,
+                                   int lambda, int asymmetric, uint8_t* __restrict__ solid) {
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= (size_t)d.nx * d.ny) return;
+  const int x = (int)(q % d.nx), gy = d.gy((int)(q / d.nx));  // row of the whole lattice
+  const int m = x % lambda;
+  uint8_t v = 0;
+  const int jd = gy, ju = d.ny_glob - 1 - gy;  // rows from the bottom / top wall
+  if (down && jd < height) { const int r = cut[jd], l = asymmetric ? 0 : r; v |= (m >= l && m < width - r) ? 1 : 0; }
+  if (up && ju < height) { const int r = cut[ju], l = asymmetric ? 0 : r; v |= (m >= l && m < width - r) ? 1 : 0; }
+  solid[q] = v;
+}
+
+// ---- initial velocity perturbation (reading R29) on time-t populations in the ABI layout [9][ny][nx]
+__global__ void perturb_kernel(const Dev d, double amplitude, double* __restrict__ fA, double* __restrict__ fB) {
+  const size_t n = (size_t)d.nx * d.ny;
+  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= n || d.solid[q]) return;
+  const int x = (int)(q % d.nx), gy = d.gy((int)(q / d.nx));
+  const double pi = 3.14159265358979323846;
+  const double duy = amplitude * sin(2.0 * pi * (double)x / (double)d.nx) * sin(pi * ((double)gy + 0.5) / (double)d.ny_glob);
+  double ra = 0.0, rb = 0.0;
+#pragma unroll
+  for (int i = 0; i < 9; i++) { ra += fA[i * n + q]; rb += fB[i * n + q]; }
+#pragma unroll
+  for (int i = 0; i < 9; i++) {
+    const double cu = (double)cy(i) * duy;
+    fA[i * n + q] += 3.0 * wq(i) * ra * cu;
+    fB[i * n + q] += 3.0 * wq(i) * rb * cu;
+  }
+}
+
 // ---- y-slab halo rows (tlb.h "Y-SLABS"): the kHalo owned rows next to a face <-> a contiguous buffer
 // [27][kHalo][px] (whole padded rows, ghost columns included).  face 0 = low y, 1 = high y.
 // pack reads the owned rows next to the face; unpack writes the halo rows beyond it.
@@ -449,6 +482,15 @@ int launch_halo_unpack(const Dev& d, void* S, int face, const void* buf, cudaStr
   const long long n = 27ll * kHalo * d.px;
   if (d.prec == 32) halo_copy_kernel<true, float><<<blocks_for(n, 256), 256, 0, st>>>(d, static_cast<float*>(S), face, const_cast<float*>(static_cast<const float*>(buf)));
   else halo_copy_kernel<true, double><<<blocks_for(n, 256), 256, 0, st>>>(d, static_cast<double*>(S), face, const_cast<double*>(static_cast<const double*>(buf)));
+  return 1;
+}
+int launch_rough_walls(const Dev& d, const int* cut, int height, int up, int down, int width, int lambda, int asymmetric,
+                       uint8_t* solid, cudaStream_t st) {
+  rough_walls_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, cut, height, up, down, width, lambda, asymmetric, solid);
+  return 1;
+}
+int launch_perturb(const Dev& d, double amplitude, double* fA, double* fB, cudaStream_t st) {
+  perturb_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, amplitude, fA, fB);
   return 1;
 }
 int launch_label_init(const Dev& d, const double* rhoA, double threshold, int* labels, cudaStream_t st) {

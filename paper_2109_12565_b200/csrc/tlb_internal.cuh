@@ -142,6 +142,9 @@ int launch_t1(const int* past, int n_past, const int* now, int n_now, const int*
               int max_events, int* n_events, int* events, cudaStream_t st);
 int launch_droplet_nusselt(const Dev& d, const double* uy, const double* T, const double* centres, int n, double tau_g,
                            double* nu, cudaStream_t st);
+int launch_rough_walls(const Dev& d, const int* cut, int height, int up, int down, int width, int lambda, int asymmetric,
+                       uint8_t* solid, cudaStream_t st);
+int launch_perturb(const Dev& d, double amplitude, double* fA, double* fB, cudaStream_t st);
 int configure_kernels();  // opt in to the dynamic shared memory the fused kernel needs; 0 on success
 int default_seg_rows(int nx, int ny);
 
