@@ -169,14 +169,12 @@ struct Smem {
   double psi[kWarps][kRingRows][kWR][2];     //           {psi^s_A, psi^s_B}          a half-warp 128: conflict-free)
   uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
   uint64_t full[kSlots];                     // mbarriers: row landed
-  unsigned int done[kSlots];                 // warps that have finished reading the slot (running count)
+  uint64_t empty[kSlots];                    // mbarriers: all kWarps warps have finished reading the slot
 };
 
-// acq_rel arrive on a shared counter; returns the previous value
-__device__ __forceinline__ unsigned int count_out(unsigned int* c) {
-  unsigned int old;
-  asm volatile("atom.acq_rel.cta.shared.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(c)) : "memory");
-  return old;
+// release arrive of one thread on an mbarrier (the warp is done with the slot the barrier guards)
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ double pair(double v) { return __shfl_xor_sync(0xffffffffu, v, 1); }  // the other species' lane
 
@@ -228,7 +226,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 
   if (t == 0) {
 #pragma unroll
-    for (int i = 0; i < kSlots; i++) { mbar_init(&sm.full[i], 1); sm.done[i] = 0; }
+    for (int i = 0; i < kSlots; i++) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], kWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -328,6 +326,30 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     const int y = r - 2;        // row of phase 2
     const bool do2 = y >= y0;
     if (do2 && (MODE == 1 || MODE == 3 || d.thermal)) load_g(y);  // consumed after the force stencil (a row earlier measured slower)
+    // Re-arm the slot every warp left during the previous iteration (row q - 3) with row q + 1, one iteration ahead of its
+    // use; the warps take turns, and by now the others have long passed their arrive, so the wait does not spin.
+    if (q >= 3 && wid == ((q - 1) & (kWarps - 1)) && lane == 0) {
+      mbar_wait(&sm.empty[(q + 1) & 3], ((q - 3) >> 2) & 1u);
+      if (q + 1 < q_end) issue(q + 1);
+      const int yp = y0 + q - 4 + kGPrefetchRows;  // phase 2 of row yp runs kGPrefetchRows iterations from now
+      if ((MODE == 1 || MODE == 3 || d.thermal) && yp < y1) {
+        int ym = yp - 1, yq = yp + 1;
+        if (PERIODIC) {
+          if (ym < 0) ym = ny - 1;
+          if (yq >= ny) yq = 0;
+        }
+        if (kTensor && (!PERIODIC || (yp > 0 && yp < ny - 1))) {
+          tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp + 2, 0, 0);
+        } else {
+          const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
+#pragma unroll
+          for (int i = 0; i < 9; i++) {
+            const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
+            prefetch_l2(Sin + (18 + pslot(i)) * plane + o, kCopyW * kB);
+          }
+        }
+      }
+    }
     // ---- (1) rho_s, psi^s_s of row r (Eqs. (4), (12)); wall values at solid / out-of-domain nodes (L155, R9)
     if (valid) {
       mbar_wait(&sm.full[slot], (parity >> slot) & 1u);
@@ -360,27 +382,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       for (int i = 0; i < 9; i++) f[i] = (double)fs[pslot(i) * kSW - cx(i)];
     }
     __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
-    if (lane == 0 && q >= 2 && (count_out(&sm.done[slot2]) & (kWarps - 1)) == kWarps - 1) {  // last warp out: the slot is free
-      if (q + 2 < q_end) issue(q + 2);
-      const int yp = y0 + q - 4 + kGPrefetchRows;  // phase 2 of row yp runs kGPrefetchRows iterations from now
-      if ((MODE == 1 || MODE == 3 || d.thermal) && yp < y1) {
-        int ym = yp - 1, yq = yp + 1;
-        if (PERIODIC) {
-          if (ym < 0) ym = ny - 1;
-          if (yq >= ny) yq = 0;
-        }
-        if (kTensor && (!PERIODIC || (yp > 0 && yp < ny - 1))) {
-          tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp + 2, 0, 0);
-        } else {
-          const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
-#pragma unroll
-          for (int i = 0; i < 9; i++) {
-            const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-            prefetch_l2(Sin + (18 + pslot(i)) * plane + o, kCopyW * kB);
-          }
-        }
-      }
-    }
+    if (lane == 0 && q >= 2) mbar_arrive(&sm.empty[slot2]);
     if (!do2) continue;
 
     // ---- (2) collide row y = r - 2, whose stencil rows y-2..y+2 = r-4..r are resident
