@@ -181,7 +181,7 @@ bool make_maps(tlb_handle* h) {
   const cuuint64_t B = sizeof(double);
   const cuuint64_t row = (cuuint64_t)d.row * B, plane = (cuuint64_t)d.plane * B;
   const cuuint64_t dims[5] = {(cuuint64_t)d.px, (cuuint64_t)d.ny + 2, 3, 3, 2};
-  const cuuint64_t strides[4] = {row, plane, 3 * plane - row, 9 * plane};  // bytes, dimensions 1..4
+  const cuuint64_t strides[4] = {row, plane, 3 * plane + row, 9 * plane};  // bytes, dimensions 1..4
   const cuuint32_t box[5] = {(cuuint32_t)kCopyW, 1, 3, 3, 2};
   const cuuint32_t ones[5] = {1, 1, 1, 1, 1};
   for (int k = 0; k < 2; k++) {
@@ -396,8 +396,11 @@ static int create_common(int nx, int ny_glob, int y0, int y1, bool slab, const t
   d.wall_hi = (!p->periodic_y && g.halo_hi == 0) ? 1 : 0;
   d.px = padded_pitch(nx);
   d.prec = p->pop_precision == 32 ? 32 : 64;
-  d.plane = (long long)d.px * (ny + 2);
-  d.row = d.px;
+  // row-interleaved planes: the 27 plane rows of one lattice row lie next to one another ([ny + 2][27][px]), so the
+  // rows a CTA works on sit in a few MB instead of being spread over 27 planes of the whole buffer (same-box A/B on
+  // config 4 against plane-major [27][ny + 2][px]: 0.674 -> 0.652 ms)
+  d.plane = d.px;
+  d.row = 27ll * d.px;
   d.omega = 1.0 / p->tau; d.omega_g = 1.0 / p->tau_g; d.tau = p->tau;
   d.rho0 = p->rho0; d.inv_rho0 = 1.0 / p->rho0;
   d.G12 = p->G12; d.G11a = p->G11a; d.G11r = p->G11r; d.G22a = p->G22a; d.G22r = p->G22r;

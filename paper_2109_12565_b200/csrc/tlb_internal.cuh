@@ -12,13 +12,15 @@
 //   * ghost columns x = -kGhost..-1 and nx..nx+kGhost-1 hold the periodic images S(x -+ nx) (the
 //     paper's own ghost-node device, footnote 2 L180); every kernel that writes column x also
 //     writes its images, so no separate halo-refresh pass exists.
-// A plane is [ny + 2][px] doubles, x fastest, lattice column x at offset kXL + x within a row; px
+// A buffer is [ny + 2][27][px] doubles: x fastest, then the 27 planes of one row, then the rows ("row-interleaved
+// planes"; Dev.plane = px and Dev.row = 27 px are the strides, and nothing but tlb_create fixes them); lattice column
+// x sits at offset kXL + x within a plane row; px
 // and kXL are multiples of 16 doubles so that x = 0 of every row starts a 128-byte line and the
 // strip copies of the fused kernel are 16-byte aligned.  27 planes per buffer: [0, 9) f_A, [9, 18) f_B,
 // [18, 27) g; inside a set the planes are ordered by c_y (pslot() below): the three directions with
-// c_y = -1, then c_y = 0, then c_y = +1.  A target row r pulls storage row (r + 1) - c_y of plane i, so
+// c_y = +1, then c_y = 0, then c_y = -1.  A target row r pulls storage row (r + 1) - c_y of plane i, so
 // with this order ONE tensor-map copy (cp.async.bulk.tensor, box x * 1 row * 3 planes * 3 groups * 2 species,
-// group stride = 3 planes - 1 row) brings the 18 fluid plane rows of a strip, already shifted in y.
+// group stride = 3 planes + 1 row) brings the 18 fluid plane rows of a strip, already shifted in y.
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
@@ -36,7 +38,7 @@ __host__ __device__ constexpr int cy(int i) { return i == 2 || i == 5 || i == 6 
 __host__ __device__ constexpr int opp(int i) { return i == 0 ? 0 : (i <= 4 ? ((i + 1) % 4) + 1 : ((i - 3) % 4) + 5); }
 // plane of direction i inside its set (internal order, see above); the ABI keeps the order R1
 __host__ __device__ constexpr int pslot(int i) {
-  return i == 4 ? 0 : i == 7 ? 1 : i == 8 ? 2 : i == 0 ? 3 : i == 1 ? 4 : i == 3 ? 5 : i == 2 ? 6 : i == 5 ? 7 : 8;
+  return i == 2 ? 0 : i == 5 ? 1 : i == 6 ? 2 : i == 0 ? 3 : i == 1 ? 4 : i == 3 ? 5 : i == 4 ? 6 : i == 7 ? 7 : 8;
 }
 __host__ __device__ constexpr double wq(int i) { return i == 0 ? 4.0 / 9.0 : (i <= 4 ? 1.0 / 9.0 : 1.0 / 36.0); }
 
@@ -96,9 +98,9 @@ struct FusedOut {
 };
 
 // Tensor maps of one fp64 population buffer (built by tlb_create with cuTensorMapEncodeTiled):
-//   f: 5-D (x, row, plane-in-group 3, c_y group 3, species 2), strides (1, row, plane, 3 plane - row, 9 plane);
+//   f: 5-D (x, row, plane-in-group 3, c_y group 3, species 2), strides (1, row, plane, 3 plane + row, 9 plane);
 //   g: 4-D, the same without the species dimension, based at plane 18.
-// Row coordinate r + 2 addresses, in group k (c_y = k - 1), storage row r + 2 - k = (r + 1) - c_y.
+// Row coordinate r addresses, in group k (c_y = 1 - k), storage row r + k = (r + 1) - c_y.
 struct TMaps {
   CUtensorMap f, g;
 };

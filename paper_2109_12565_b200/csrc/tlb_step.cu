@@ -23,6 +23,10 @@
 // last warp out issues the copy of row r+2 into that slot, a full row of compute ahead of its use.
 #include "tlb_internal.cuh"
 
+#ifndef TLB_LEAD1
+#define TLB_LEAD1 1
+#endif
+
 namespace tlb {
 
 namespace {
@@ -162,9 +166,16 @@ constexpr int kWR = kWC + 4;           // ring columns per warp: its 16 columns 
 template <typename ST> struct SlotW { static constexpr int v = kCopyW; };
 template <> struct SlotW<float> { static constexpr int v = kCopyW + 8; };
 
-template <typename ST>
+// TAU1 (tau = 1, the time step only): the collision needs rho_l, j and F of a site, not its populations, so phase 1
+// also leaves the momentum of its row in a small ring and a landed row is dead after phase 1: 3 slots instead of 4,
+// and phase 2 reads one 16-byte pair instead of 9 populations.  Phase 2 then runs THREE rows behind phase 1, so that
+// inside one iteration the two phases touch disjoint ring rows and are independent: they sit in one basic block
+// (phase 1 is branch-free there) and the compiler interleaves their dependency chains.
+template <typename ST, bool TAU1>
 struct Smem {
-  ST f[kSlots][18][SlotW<ST>::v];            // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
+  static constexpr int kS = TAU1 ? 3 : kSlots;
+  ST f[kS][18][SlotW<ST>::v];                // landed rows of f_A, f_B (columns x0 - kHX .. x0 + kW + kHX - 1)
+  double2 jr[TAU1 ? kWarps : 1][TAU1 ? 4 : 1][kWC][2];  // TAU1: per warp, 4 rows of {j_x, j_y} of (column, species)
   double rho[kWarps][kRingRows][kWR][2];     // per warp: {rho_A, rho_B} per column (a lane pair reads 16 contiguous bytes,
   double psi[kWarps][kRingRows][kWR][2];     //           {psi^s_A, psi^s_B}          a half-warp 128: conflict-free)
   uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
@@ -198,7 +209,7 @@ __device__ __forceinline__ double relax_tau1(double owd, double cu, double usq) 
 // (phase 1), its force, shifted velocity, collision and 9 stores (phase 2) -- and half of the thermal
 // set: s = 0 takes g_0, g_1, g_2, g_5, g_6, s = 1 the opposite directions g_3, g_4, g_7, g_8, so both
 // lanes run the same code on (c_i, u) and (-c_i, -u).  Partial sums (j, F, T) cross by one shuffle.
-template <int MODE, bool PERIODIC, typename ST>
+template <int MODE, bool PERIODIC, typename ST, bool TAU1>
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
 fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int seg_rows, int ya, int yb,
              const FusedOut out, const __grid_constant__ TMaps tm) {
@@ -209,8 +220,11 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
   double* __restrict__ const oUy = out.uy;
   double* __restrict__ const oT = out.T;
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  Smem<ST>& sm = *reinterpret_cast<Smem<ST>*>(smem_raw);
-  constexpr int kSW = SlotW<ST>::v, kB = (int)sizeof(ST);
+  using SmemT = Smem<ST, TAU1>;
+  SmemT& sm = *reinterpret_cast<SmemT*>(smem_raw);
+  constexpr int kSW = SlotW<ST>::v, kB = (int)sizeof(ST), kS = SmemT::kS;
+  static_assert(!TAU1 || MODE == 0, "the tau = 1 path is the time step only");
+  auto slot_of = [](int q) { return TAU1 ? q % 3 : q & 3; };
 
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const int k = lane >> 1, s = lane & 1;
@@ -226,7 +240,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 
   if (t == 0) {
 #pragma unroll
-    for (int i = 0; i < kSlots; i++) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], kWarps); }
+    for (int i = 0; i < kS; i++) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], kWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -244,11 +258,12 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       if (rm < 0) rm = ny - 1;
       if (rp >= ny) rp = 0;
     }
-    uint64_t* bar = &sm.full[q & 3];
+    const int sl = slot_of(q);
+    uint64_t* bar = &sm.full[sl];
     mbar_expect_tx(bar, 18u * kCopyW * kB);
     if (kTensor && (!PERIODIC || (rr > 0 && rr < ny - 1))) {
       // one copy: box 136 x 1 x 3 x 3 x 2 = the 18 fluid plane rows, each shifted by its c_y (tlb_internal.cuh)
-      tma_g2s_5d(&sm.f[q & 3][0][0], &tm.f, kXL + x0 - kHX, rr + 2, 0, 0, 0, bar, pol);
+      tma_g2s_5d(&sm.f[sl][0][0], &tm.f, kXL + x0 - kHX, rr, 0, 0, 0, bar, pol);
       return;
     }
     const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
@@ -257,11 +272,11 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 #pragma unroll
       for (int i = 0; i < 9; i++) {
         const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-        bulk_g2s(&sm.f[q & 3][l * 9 + pslot(i)][0], Sin + (l * 9 + pslot(i)) * plane + o, kCopyW * kB, bar, pol);
+        bulk_g2s(&sm.f[sl][l * 9 + pslot(i)][0], Sin + (l * 9 + pslot(i)) * plane + o, kCopyW * kB, bar, pol);
       }
   };
   if (t == 0) {
-    for (int q = 0; q < 4 && q < q_end; q++) issue(q);
+    for (int q = 0; q < (TAU1 ? TLB_LEAD1 : kS) && q < q_end; q++) issue(q);
   }
 
   // phase-1 tasks of this lane: ring column k and, for lanes < 8, ring column 16 + k; species s
@@ -288,11 +303,11 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 
   // running byte pointers of row y = y0 (advanced by one row per phase-2 iteration)
   // thermal planes of lane s (internal order pslot()): g_0 at plane 3 (lane 0 only), g_1 / g_3 at 4 + s,
-  // {g_2, g_5, g_6} at 6, 7, 8 (lane 0), {g_4, g_7, g_8} at 0, 1, 2 (lane 1): 6 planes lower
+  // {g_2, g_5, g_6} at 0, 1, 2 (lane 0), {g_4, g_7, g_8} at 6, 7, 8 (lane 1): 6 planes higher
   const char* gp = reinterpret_cast<const char*>(Sin + (18 + s) * plane + d.at(x, y0));
   char* opf = reinterpret_cast<char*>(Sout + 9 * s * plane + d.at(x, y0));                    // own species
   char* opg = reinterpret_cast<char*>(Sout + (18 + s) * plane + d.at(x, y0));                 // own thermal half
-  const long long sofs = s ? -7 * planeB : 0;                                                    // planes 6.. -> 0.. for lane 1
+  const long long sofs = s ? 5 * planeB : 0;                                                     // planes 0.. -> 6.. for lane 1 (gp, opg carry + s)
   const int co = s ? kB : -kB;                                                                    // x - c_x of c_1 / c_3
 
   // thermal populations of (x, y).  Lane s = 0 reads
@@ -308,30 +323,42 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     rofs += sofs;
     g0 = ldg_stream(reinterpret_cast<const ST*>(gp + 3 * planeB), pol);  // lane 1 reads g_1 here and never uses it
     ga = ldg_stream(reinterpret_cast<const ST*>(gp + 4 * planeB + co), pol);
-    gb = ldg_stream(reinterpret_cast<const ST*>(gp + 6 * planeB + rofs), pol);
-    gc = ldg_stream(reinterpret_cast<const ST*>(gp + 7 * planeB + rofs + co), pol);
-    gd = ldg_stream(reinterpret_cast<const ST*>(gp + 8 * planeB + rofs - co), pol);
+    gb = ldg_stream(reinterpret_cast<const ST*>(gp + rofs), pol);
+    gc = ldg_stream(reinterpret_cast<const ST*>(gp + 1 * planeB + rofs + co), pol);
+    gd = ldg_stream(reinterpret_cast<const ST*>(gp + 2 * planeB + rofs - co), pol);
   };
 
+  constexpr int kLag = TAU1 ? 3 : 2;  // rows between phase 1 and phase 2
   uint32_t parity = 0;  // one bit per slot
-  for (int q = 0; q < q_end; q++) {
+  for (int q = 0; q < q_end + (kLag - 2); q++) {
     const int r = y0 - 2 + q;
-    const int slot = q & 3, rq = q % kRingRows;
-    const bool valid = row_valid(r);
+    const int slot = slot_of(q), rq = q % kRingRows;
+    const bool p1 = q < q_end;  // phase 1 has a row (TAU1 runs one more iteration for the last phase 2)
+    const bool valid = p1 && row_valid(r);
     const uint8_t s0 = m0, s1 = m1;
     if (q + 1 < q_end) {  // mask of the next row, a full iteration ahead of its use
       m0 = mask_at(r + 1, k);
       if (extra) m1 = mask_at(r + 1, kWC + k);
     }
-    const int y = r - 2;        // row of phase 2
+    const int y = r - kLag;     // row of phase 2
     const bool do2 = y >= y0;
     if (do2 && (MODE == 1 || MODE == 3 || d.thermal)) load_g(y);  // consumed after the force stencil (a row earlier measured slower)
     // Re-arm the slot every warp left during the previous iteration (row q - 3) with row q + 1, one iteration ahead of its
     // use; the warps take turns, and by now the others have long passed their arrive, so the wait does not spin.
-    if (q >= 3 && wid == ((q - 1) & (kWarps - 1)) && lane == 0) {
-      mbar_wait(&sm.empty[(q + 1) & 3], ((q - 3) >> 2) & 1u);
-      if (q + 1 < q_end) issue(q + 1);
-      const int yp = y0 + q - 4 + kGPrefetchRows;  // phase 2 of row yp runs kGPrefetchRows iterations from now
+    // (TAU1: a slot is left right after phase 1 of its row; row q + kLead1 goes into the slot of row q + kLead1 - 3.)
+    constexpr int kLead1 = TLB_LEAD1;
+    if (q >= (TAU1 ? 0 : 3) && wid == ((q - 1) & (kWarps - 1)) && lane == 0) {
+      if (TAU1) {
+        const int qi = q + kLead1;
+        if (qi < q_end) {
+          if (qi >= 3) mbar_wait(&sm.empty[slot_of(qi)], ((qi - 3) / 3) & 1u);
+          issue(qi);
+        }
+      } else {
+        mbar_wait(&sm.empty[(q + 1) & 3], ((q - 3) >> 2) & 1u);
+        if (q + 1 < q_end) issue(q + 1);
+      }
+      const int yp = y0 + q - 2 - kLag + kGPrefetchRows;  // phase 2 of row yp runs kGPrefetchRows iterations from now
       if ((MODE == 1 || MODE == 3 || d.thermal) && yp < y1) {
         int ym = yp - 1, yq = yp + 1;
         if (PERIODIC) {
@@ -339,7 +366,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
           if (yq >= ny) yq = 0;
         }
         if (kTensor && (!PERIODIC || (yp > 0 && yp < ny - 1))) {
-          tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp + 2, 0, 0);
+          tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp, 0, 0);
         } else {
           const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
 #pragma unroll
@@ -355,6 +382,33 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       mbar_wait(&sm.full[slot], (parity >> slot) & 1u);
       parity ^= 1u << slot;
     }
+    if (TAU1) {
+      // branch-free: every lane runs both passes (lanes >= 8 redo a halo column in the second and store nothing), solid
+      // and out-of-domain nodes take the wall values by selection, so that phases 1 and 2 share one basic block
+      if (p1) {
+#pragma unroll
+        for (int pass = 0; pass < 2; pass++) {
+          const int c = pass == 0 ? k : kWC + (k & 3);
+          const bool act = pass == 0 || extra;
+          const uint8_t sol = pass == 0 ? s0 : s1;
+          const ST* fs = &sm.f[slot][9 * s][kWC * wid + c + 2];  // S(x) of ring column c
+          double f[9];
+#pragma unroll
+          for (int i = 0; i < 9; i++) f[i] = (double)fs[pslot(i) * kSW - cx(i)];
+          const double rc = sum9(f);
+          const double pc = d.rho0 * (1.0 - exp_nonpos(-rc * d.inv_rho0));
+          const double rl = sol ? rho_wall : rc, pl = sol ? pss_wall : pc;
+          if (act) {
+            rho_r[rq][c][s] = rl;
+            psi_r[rq][c][s] = pl;
+            flag[rq][c] = sol;
+            if (c >= 2 && c < kWC + 2)  // an interior column: its momentum, Eq. (5), for phase 2 three rows later
+              sm.jr[wid][q & 3][c - 2][s] = make_double2(((f[1] - f[3]) + (f[5] - f[6])) + (f[8] - f[7]),
+                                                         ((f[2] - f[4]) + (f[5] - f[7])) + (f[6] - f[8]));
+          }
+        }
+      }
+    } else {
 #pragma unroll
     for (int pass = 0; pass < 2; pass++) {
       if (pass == 1 && !extra) break;
@@ -373,20 +427,23 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       psi_r[rq][c][s] = pl;
       flag[rq][c] = sol;
     }
+    }
     // the 9 own-species populations of (x, y), landed two iterations ago
     const int slot2 = (q + 2) & 3;  // == (q - 2) & 3
     double f[9];
-    {
+    if (!TAU1) {
       const ST* fs = &sm.f[slot2][9 * s][kWC * wid + k + kHX];
 #pragma unroll
       for (int i = 0; i < 9; i++) f[i] = (double)fs[pslot(i) * kSW - cx(i)];
     }
-    __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
-    if (lane == 0 && q >= 2) mbar_arrive(&sm.empty[slot2]);
-    if (!do2) continue;
+    if (!TAU1) {
+      __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
+      if (lane == 0 && q >= 2) mbar_arrive(&sm.empty[slot2]);
+    }
+    if (do2) {
 
     // ---- (2) collide row y = r - 2, whose stencil rows y-2..y+2 = r-4..r are resident
-    const int rq0 = (q + kRingRows - 2) % kRingRows;  // ring row of y
+    const int rq0 = (q + kRingRows - kLag) % kRingRows;  // ring row of y
     const int cc = k + 2;                             // ring column of x
     const bool fluid = x < nx && !flag[rq0][cc];
     const double rl = rho_r[rq0][cc][s], rn = rho_r[rq0][cc][1 - s], pl = psi_r[rq0][cc][s];
@@ -396,7 +453,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     double Xx = 0, Xy = 0, Sx = 0, Sy = 0, Sx2 = 0, Sy2 = 0;  // S = S + S2: two dependency chains per component
 #pragma unroll
     for (int dy = 0; dy <= 2; dy++) {
-      const int slp = (q + kRingRows - 2 + dy) % kRingRows, slm = (q + kRingRows - 2 - dy) % kRingRows;
+      const int slp = (q + kRingRows - kLag + dy) % kRingRows, slm = (q + 2 * kRingRows - kLag - dy) % kRingRows;
 #pragma unroll
       for (int dx = -2; dx <= 2; dx++) {
         if (dy == 0 && dx <= 0) continue;  // one representative of every pair {c, -c}
@@ -422,8 +479,15 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     // moments, Eqs. (5), (17): partial sums of this lane + the other species' lane
     const double Tp = (s ? 0.0 : g0) + ga + gb + gc + gd;
     const double T = Tp + pair(Tp);
-    const double jxl = ((f[1] - f[3]) + (f[5] - f[6])) + (f[8] - f[7]);
-    const double jyl = ((f[2] - f[4]) + (f[5] - f[7])) + (f[6] - f[8]);
+    double jxl, jyl;
+    if (TAU1) {
+      const double2 jl = sm.jr[wid][(q + 1) & 3][k][s];  // row y = r - 3: written three iterations ago
+      jxl = jl.x;
+      jyl = jl.y;
+    } else {
+      jxl = ((f[1] - f[3]) + (f[5] - f[6])) + (f[8] - f[7]);
+      jyl = ((f[2] - f[4]) + (f[5] - f[7])) + (f[6] - f[8]);
+    }
     const double jx = jxl + pair(jxl), jy = jyl + pair(jyl);
     // Eq. (22) buoyancy (R12) and the x-acceleration extension
     const double dT = d.thermal ? (T - d.T_ref) : 0.0;
@@ -453,7 +517,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       // a10: mass_l (north_star), E (L248, R11), Nu (Eq. (24), R10).  R10's face differences telescope over every
       // fluid-fluid link, so sum_fluid d_y T = sum over fluid sites of [solid above] T_w(y + 1) - [solid below] T_w(y - 1).
       if (fluid) {
-        const int rqp = (q + kRingRows - 1) % kRingRows, rqm = (q + kRingRows - 3) % kRingRows;  // ring rows of y + 1, y - 1
+        const int rqp = (q + kRingRows - kLag + 1) % kRingRows, rqm = (q + kRingRows - kLag - 1) % kRingRows;  // ring rows of y + 1, y - 1
         int yu = y + 1, yd = y - 1;
         if (PERIODIC) { yu = yu >= ny ? 0 : yu; yd = yd < 0 ? ny - 1 : yd; }
         acc0 += rl;
@@ -467,13 +531,13 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       }
     } else {
       // kinetic part of P_xy (R21): momentum flux sum_i c_ix c_iy f_i of the populations arriving at (x, y) ...
-      const double kpre = (f[5] - f[6]) + (f[7] - f[8]);
+      const double kpre = TAU1 ? 0.0 : (f[5] - f[6]) + (f[7] - f[8]);
       // own species: Eq. (6) shifted velocity, Eqs. (2), (3)
       {
         const double vx = ux + Fx * invl, vy = uy + Fy * invl;
         const double usq = 1.0 - 1.5 * (vx * vx + vy * vy);
         const double w0 = d.omega * (wq(0) * rl), w1 = d.omega * (wq(1) * rl), w5 = d.omega * (wq(5) * rl);
-        if (om1 == 0.0) {  // uniform branch
+        if (TAU1 || om1 == 0.0) {  // uniform branch
           f[0] = relax_tau1(w0, 0.0, usq);
           f[1] = relax_tau1(w1, vx, usq);
           f[2] = relax_tau1(w1, vy, usq);
@@ -503,7 +567,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
         double Is = 0.0, Ix = 0.0;
 #pragma unroll
         for (int dy = 1; dy <= 2; dy++) {
-          const int slp = (q + kRingRows - 2 + dy) % kRingRows, slm = (q + kRingRows - 2 - dy) % kRingRows;
+          const int slp = (q + kRingRows - kLag + dy) % kRingRows, slm = (q + 2 * kRingRows - kLag - dy) % kRingRows;
 #pragma unroll
           for (int dx = -2; dx <= 2; dx++) {
             if (dx == 0) continue;
@@ -542,9 +606,9 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
         if (d.thermal) {
           if (!s) stg_stream(reinterpret_cast<ST*>(opg + 3 * planeB), g0, pol);
           stg_stream(reinterpret_cast<ST*>(opg + 4 * planeB), ga, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 6 * planeB + sofs), gb, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 7 * planeB + sofs), gc, pol);
-          stg_stream(reinterpret_cast<ST*>(opg + 8 * planeB + sofs), gd, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + sofs), gb, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 1 * planeB + sofs), gc, pol);
+          stg_stream(reinterpret_cast<ST*>(opg + 2 * planeB + sofs), gd, pol);
         }
         if (x < kGhost || x >= nx - kGhost) {  // periodic images of this column (ghost columns)
           for (int pass = 0; pass < 2; pass++)
@@ -555,9 +619,9 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
               if (d.thermal) {
                 if (!s) *reinterpret_cast<ST*>(opg + 3 * planeB + e) = (ST)g0;
                 *reinterpret_cast<ST*>(opg + 4 * planeB + e) = (ST)ga;
-                *reinterpret_cast<ST*>(opg + 6 * planeB + sofs + e) = (ST)gb;
-                *reinterpret_cast<ST*>(opg + 7 * planeB + sofs + e) = (ST)gc;
-                *reinterpret_cast<ST*>(opg + 8 * planeB + sofs + e) = (ST)gd;
+                *reinterpret_cast<ST*>(opg + sofs + e) = (ST)gb;
+                *reinterpret_cast<ST*>(opg + 1 * planeB + sofs + e) = (ST)gc;
+                *reinterpret_cast<ST*>(opg + 2 * planeB + sofs + e) = (ST)gd;
               }
             }
         }
@@ -566,6 +630,11 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     gp += rowB;
     opf += rowB;
     opg += rowB;
+    }  // do2
+    if (TAU1) {
+      __syncwarp();  // ring row r of this warp is complete; this warp has read the slot of row r for the last time
+      if (lane == 0 && p1) mbar_arrive(&sm.empty[slot]);
+    }
   }
   if (MODE == 3) {
     // warp-level reduction over the 16 lanes of each species (fixed butterfly), then the 8 warps in a fixed order
@@ -657,15 +726,16 @@ static dim3 strip_grid(const Dev& d, int seg_rows, int rows) {
 
 template <typename ST>
 static cudaError_t configure_for() {
-  const int bytes = (int)sizeof(Smem<ST>);
   cudaError_t e = cudaSuccess;
-  auto set = [&](auto* k) {
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  auto set = [&](auto* k, size_t bytes) {
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
   };
-  set(fused_kernel<0, false, ST>); set(fused_kernel<0, true, ST>);
-  set(fused_kernel<1, false, ST>); set(fused_kernel<1, true, ST>);
-  set(fused_kernel<2, false, ST>); set(fused_kernel<2, true, ST>);
-  set(fused_kernel<3, false, ST>); set(fused_kernel<3, true, ST>);
+  const size_t b = sizeof(Smem<ST, false>), b1 = sizeof(Smem<ST, true>);
+  set(fused_kernel<0, false, ST, false>, b); set(fused_kernel<0, true, ST, false>, b);
+  set(fused_kernel<0, false, ST, true>, b1); set(fused_kernel<0, true, ST, true>, b1);
+  set(fused_kernel<1, false, ST, false>, b); set(fused_kernel<1, true, ST, false>, b);
+  set(fused_kernel<2, false, ST, false>, b); set(fused_kernel<2, true, ST, false>, b);
+  set(fused_kernel<3, false, ST, false>, b); set(fused_kernel<3, true, ST, false>, b);
   return e;
 }
 
@@ -710,9 +780,17 @@ static void launch_mode(const Dev& d, const void* Sin, void* Sout, int seg_rows,
   const ST* in = static_cast<const ST*>(Sin);
   ST* o = static_cast<ST*>(Sout);
   const dim3 g = strip_grid(d, seg_rows, yb - ya);
-  const size_t sm = sizeof(Smem<ST>);
-  if (d.periodic_y) fused_kernel<MODE, true, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
-  else fused_kernel<MODE, false, ST><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
+  if constexpr (MODE == 0) {
+    if (d.omega == 1.0) {  // tau = 1 (Table A.3 and every BASELINE config): the populations are not needed by the collision
+      const size_t sm1 = sizeof(Smem<ST, true>);
+      if (d.periodic_y) fused_kernel<0, true, ST, true><<<g, kThreads, sm1, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
+      else fused_kernel<0, false, ST, true><<<g, kThreads, sm1, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
+      return;
+    }
+  }
+  const size_t sm = sizeof(Smem<ST, false>);
+  if (d.periodic_y) fused_kernel<MODE, true, ST, false><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
+  else fused_kernel<MODE, false, ST, false><<<g, kThreads, sm, st>>>(d, in, o, seg_rows, ya, yb, out, tm);
 }
 
 // Launch the fused kernel in `mode` on local rows [ya, yb); returns the number of launches (0 for an empty range).
