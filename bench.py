@@ -204,7 +204,7 @@ def run_ours(args, rank, world):
     peak, peak_src = measured_peak()
     achieved = alg_bytes * sites / fused_ms / 1e6  # GB/s
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": committed_traffic(cfg["name"]) if args.pop_precision == 64 else None, "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false, double>" if args.pop_precision == 64 else "tlb::fused_kernel<0, false, float>",
+                "traffic": committed_traffic(cfg["name"]) if args.pop_precision == 64 else None, "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false, %s, %s>" % ("double" if args.pop_precision == 64 else "float", "true" if cfg["params"]["tau"] == 1.0 else "false"),
                 "kernel_ms": fused_ms, "kernel_ms_isolated": iso_ms, "boundary_kernel_ms": boundary_ms,
                 "method": "kernel_ms = ms_per_step - boundary_kernel_ms (CUDA events on the launch stream)",
                 "alg_bytes_per_launch": alg_bytes * sites, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
@@ -392,7 +392,7 @@ def run_slabs(args, rank, world, local):
     step_ms = ms / args.steps
     achieved = alg_bytes * own_sites / step_ms / 1e6  # this rank's bytes over the slowest rank's step: a lower bound
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
-                "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false, %s>" % ("double" if args.pop_precision == 64 else "float"),
+                "peak_source": peak_src, "kernel": "tlb::fused_kernel<0, false, %s, %s>" % ("double" if args.pop_precision == 64 else "float", "true" if cfg["params"]["tau"] == 1.0 else "false"),
                 "kernel_ms": step_ms, "method": "per GPU: own rows x alg. bytes / whole step time (edges + interior + halo "
                 "exchange + boundary kernel), max over ranks", "alg_bytes_per_launch": alg_bytes * own_sites}
 
