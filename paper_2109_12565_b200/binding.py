@@ -377,13 +377,14 @@ class TLB:
 
     def droplets(self, B_th, max_droplets, want_labels=True):
         """(labels [ny][nx] int32 or None, n_droplets, stats [n][4]) as device tensors / int (section 2.4, R22)."""
-        torch = self.torch
-        labels = torch.empty((self.ny, self.nx), dtype=torch.int32, device=self.device) if want_labels else None
-        n = torch.zeros(1, dtype=torch.int32, device=self.device)
-        stats = torch.zeros((max(1, max_droplets), 4), dtype=torch.float64, device=self.device)
-        self._chk(self.lib.tlb_droplets(self.h, float(B_th), _ptr(labels), int(max_droplets), n.data_ptr(), stats.data_ptr()))
-        k = int(n.item())
-        return labels, k, stats[:min(k, max_droplets)]
+        with self.torch.cuda.stream(self.stream):  # temporaries and read-backs on the stream the kernels run on
+            torch = self.torch
+            labels = torch.empty((self.ny, self.nx), dtype=torch.int32, device=self.device) if want_labels else None
+            n = torch.zeros(1, dtype=torch.int32, device=self.device)
+            stats = torch.zeros((max(1, max_droplets), 4), dtype=torch.float64, device=self.device)
+            self._chk(self.lib.tlb_droplets(self.h, float(B_th), _ptr(labels), int(max_droplets), n.data_ptr(), stats.data_ptr()))
+            k = int(n.item())
+            return labels, k, stats[:min(k, max_droplets)]
 
     def droplets_host(self, B_th, max_droplets, want_labels=True):
         torch = self.torch
@@ -397,50 +398,55 @@ class TLB:
     # ---- droplet analysis, second stage (section 2.4, R23-R26): device tensors in, device tensors out
     def voronoi(self, centres):
         """colour [ny][nx] int32: index of the nearest centre; centres [n][2] float64 device tensor."""
-        torch = self.torch
-        centres = centres.contiguous()
-        colour = torch.empty((self.ny, self.nx), dtype=torch.int32, device=self.device)
-        self._chk(self.lib.tlb_voronoi(self.h, _ptr(centres), int(centres.shape[0]), colour.data_ptr()))
-        return colour
+        with self.torch.cuda.stream(self.stream):  # temporaries and read-backs on the stream the kernels run on
+            torch = self.torch
+            centres = centres.contiguous()
+            colour = torch.empty((self.ny, self.nx), dtype=torch.int32, device=self.device)
+            self._chk(self.lib.tlb_voronoi(self.h, _ptr(centres), int(centres.shape[0]), colour.data_ptr()))
+            return colour
 
     def delaunay(self, colour, n, max_links=None):
         """(links [m][2] int32 sorted, n_links) from a colouring with n colours."""
-        torch = self.torch
-        cap = int(max_links) if max_links is not None else 16 * max(1, int(n))
-        links = torch.zeros((max(cap, 1), 2), dtype=torch.int32, device=self.device)
-        nl = torch.zeros(1, dtype=torch.int32, device=self.device)
-        self._chk(self.lib.tlb_delaunay(self.h, colour.data_ptr(), int(n), cap, nl.data_ptr(), links.data_ptr()))
-        k = int(nl.item())
-        return links[:max(0, min(k, cap))], k
+        with self.torch.cuda.stream(self.stream):  # temporaries and read-backs on the stream the kernels run on
+            torch = self.torch
+            cap = int(max_links) if max_links is not None else 16 * max(1, int(n))
+            links = torch.zeros((max(cap, 1), 2), dtype=torch.int32, device=self.device)
+            nl = torch.zeros(1, dtype=torch.int32, device=self.device)
+            self._chk(self.lib.tlb_delaunay(self.h, colour.data_ptr(), int(n), cap, nl.data_ptr(), links.data_ptr()))
+            k = int(nl.item())
+            return links[:max(0, min(k, cap))], k
 
     def droplet_match(self, colour_past, centres_now):
-        torch = self.torch
-        centres_now = centres_now.contiguous()
-        m = torch.zeros(max(1, int(centres_now.shape[0])), dtype=torch.int32, device=self.device)
-        self._chk(self.lib.tlb_droplet_match(self.h, colour_past.data_ptr(), _ptr(centres_now), int(centres_now.shape[0]),
-                                             m.data_ptr()))
-        return m[:int(centres_now.shape[0])]
+        with self.torch.cuda.stream(self.stream):  # temporaries and read-backs on the stream the kernels run on
+            torch = self.torch
+            centres_now = centres_now.contiguous()
+            m = torch.zeros(max(1, int(centres_now.shape[0])), dtype=torch.int32, device=self.device)
+            self._chk(self.lib.tlb_droplet_match(self.h, colour_past.data_ptr(), _ptr(centres_now), int(centres_now.shape[0]),
+                                                 m.data_ptr()))
+            return m[:int(centres_now.shape[0])]
 
     def t1_events(self, links_past, links_now, n_droplets, map_now_to_past=None, max_events=4096):
         """(events [e][4] int32 = (a, b, c, d): link a-b replaced by c-d, n_events)."""
-        torch = self.torch
-        links_past, links_now = links_past.contiguous(), links_now.contiguous()
-        ev = torch.zeros((max(1, max_events), 4), dtype=torch.int32, device=self.device)
-        ne = torch.zeros(1, dtype=torch.int32, device=self.device)
-        mp = map_now_to_past.contiguous() if map_now_to_past is not None else None
-        self._chk(self.lib.tlb_t1_events(self.h, _ptr(links_past), int(links_past.shape[0]), _ptr(links_now),
-                                         int(links_now.shape[0]), _ptr(mp), 0 if mp is None else int(mp.shape[0]),
-                                         int(n_droplets), int(max_events), ne.data_ptr(), ev.data_ptr()))
-        k = int(ne.item())
-        return ev[:max(0, min(k, max_events))], k
+        with self.torch.cuda.stream(self.stream):  # temporaries and read-backs on the stream the kernels run on
+            torch = self.torch
+            links_past, links_now = links_past.contiguous(), links_now.contiguous()
+            ev = torch.zeros((max(1, max_events), 4), dtype=torch.int32, device=self.device)
+            ne = torch.zeros(1, dtype=torch.int32, device=self.device)
+            mp = map_now_to_past.contiguous() if map_now_to_past is not None else None
+            self._chk(self.lib.tlb_t1_events(self.h, _ptr(links_past), int(links_past.shape[0]), _ptr(links_now),
+                                             int(links_now.shape[0]), _ptr(mp), 0 if mp is None else int(mp.shape[0]),
+                                             int(n_droplets), int(max_events), ne.data_ptr(), ev.data_ptr()))
+            k = int(ne.item())
+            return ev[:max(0, min(k, max_events))], k
 
     def droplet_nusselt(self, centres):
         """Nu_i of Eq. (25) [n] at the sites nearest to the centres [n][2]."""
-        torch = self.torch
-        centres = centres.contiguous()
-        nu = torch.zeros(max(1, int(centres.shape[0])), dtype=torch.float64, device=self.device)
-        self._chk(self.lib.tlb_droplet_nusselt(self.h, _ptr(centres), int(centres.shape[0]), nu.data_ptr()))
-        return nu[:int(centres.shape[0])]
+        with self.torch.cuda.stream(self.stream):  # temporaries and read-backs on the stream the kernels run on
+            torch = self.torch
+            centres = centres.contiguous()
+            nu = torch.zeros(max(1, int(centres.shape[0])), dtype=torch.float64, device=self.device)
+            self._chk(self.lib.tlb_droplet_nusselt(self.h, _ptr(centres), int(centres.shape[0]), nu.data_ptr()))
+            return nu[:int(centres.shape[0])]
 
     def seg_rows(self):
         return int(self.lib.tlb_seg_rows(self.h))

@@ -23,10 +23,6 @@
 // last warp out issues the copy of row r+2 into that slot, a full row of compute ahead of its use.
 #include "tlb_internal.cuh"
 
-#ifndef TLB_LEAD1
-#define TLB_LEAD1 1
-#endif
-
 namespace tlb {
 
 namespace {
@@ -276,7 +272,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       }
   };
   if (t == 0) {
-    for (int q = 0; q < (TAU1 ? TLB_LEAD1 : kS) && q < q_end; q++) issue(q);
+    for (int q = 0; q < (TAU1 ? 1 : kS) && q < q_end; q++) issue(q);
   }
 
   // phase-1 tasks of this lane: ring column k and, for lanes < 8, ring column 16 + k; species s
@@ -345,8 +341,9 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     if (do2 && (MODE == 1 || MODE == 3 || d.thermal)) load_g(y);  // consumed after the force stencil (a row earlier measured slower)
     // Re-arm the slot every warp left during the previous iteration (row q - 3) with row q + 1, one iteration ahead of its
     // use; the warps take turns, and by now the others have long passed their arrive, so the wait does not spin.
-    // (TAU1: a slot is left right after phase 1 of its row; row q + kLead1 goes into the slot of row q + kLead1 - 3.)
-    constexpr int kLead1 = TLB_LEAD1;
+    // (TAU1: a slot is left when the iteration of its row ends; row q + 1 goes into the slot of row q - 2, free for a whole
+    // iteration.  Two rows ahead measured 8 % slower: the issuer then waits for the slowest warp of the previous row.)
+    constexpr int kLead1 = 1;
     if (q >= (TAU1 ? 0 : 3) && wid == ((q - 1) & (kWarps - 1)) && lane == 0) {
       if (TAU1) {
         const int qi = q + kLead1;

@@ -235,8 +235,11 @@ def test_profile_step_advances_exactly_one_step(tlbmod, oracle_mod):
         assert _maxdiff(o, t) <= TOL
 
 
-def test_full_size_windows_config4(tlbmod, oracle_mod):
-    """BASELINE config 4 at full size (4096x2048, posts, 4000 droplets) in the launch configuration bench.py
+@pytest.mark.parametrize("tau", [1.0, 0.9])
+def test_full_size_windows_config4(tlbmod, oracle_mod, tau):
+    """tau = 1 runs the kernel instantiation bench.py times; tau = 0.9 the general one (four slots, the populations
+    relaxed and not only their moments) in the same launch configuration.
+    BASELINE config 4 at full size (4096x2048, posts, 4000 droplets) in the launch configuration bench.py
     times: 3 steps on the GPU, compared with the oracle on windows it can compute in seconds.  A site after
     n steps depends on initial data within 3n cells (2-cell force stencil + 1 cell of streaming per step), so
     an oracle run on a window is exact farther than 3n cells from the window's artificial edges.  Windows:
@@ -244,6 +247,7 @@ def test_full_size_windows_config4(tlbmod, oracle_mod):
     segment edge, and a bulk window."""
     import torch
     cfg = inputs.config(4)
+    cfg["params"] = dict(cfg["params"], tau=tau, tau_g=tau)
     nx, ny, steps, m = cfg["nx"], cfg["ny"], 3, 12
     solid, rA, rB, T = inputs.make_config_inputs(cfg)
     t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
