@@ -742,12 +742,22 @@ int configure_kernels() {
   return e == cudaSuccess ? 0 : (int)e;
 }
 
-// Rows per CTA segment: strips x segments should fill whole waves of 2 CTAs per SM on 148 SMs with
-// as few segments as possible (each segment re-reads 4 warm-up rows), never below kMinSegRows rows
-// (small lattices are bound by the latency of the serial march, not by the redundant rows).
+// Rows per CTA segment.  strips x segments should fill whole waves of 2 CTAs per SM on 148 SMs.  Large lattices: as many
+// waves (up to 8) as keep a segment at 48 rows or more -- many short CTAs balance the SMs better than few long ones and
+// keep the rows in flight closer together, while each segment costs 4 warm-up rows and a pipeline fill (same-box
+// measurements, profiles/r02_experiments.md block K: config 3 best with 1 wave of 57-row segments, config 4 with 4 waves
+// of 56, config 5 with 8 waves of 114).  Lattices too small for that: the wave count (1..4) with the best ratio of useful
+// to marched rows, never below kMinSegRows rows (they are bound by the latency of the serial march).
 constexpr int kMinSegRows = 2;
+constexpr int kGoodSegRows = 48;
 int default_seg_rows(int nx, int ny) {
   const int strips = (nx + kW - 1) / kW, slots = kCtasPerSM * 148;
+  for (int waves = 8; waves >= 1; waves--) {
+    int segs = waves * slots / strips;
+    if (segs < 1) segs = 1;
+    const int seg = (ny + segs - 1) / segs;
+    if (seg >= kGoodSegRows) return seg;
+  }
   int best_seg = ny;
   double best = -1.0;
   for (int waves = 1; waves <= 4; waves++) {
@@ -760,7 +770,7 @@ int default_seg_rows(int nx, int ny) {
     const int w = (ctas + slots - 1) / slots;
     const double cost = (double)w * (seg + 4);  // rows marched by the busiest slot, incl. warm-up rows
     double score = (double)ny * strips / slots / cost;  // 1 = perfect
-    if (w == 1) score *= 0.97;  // a single wave cannot rebalance CTAs that run slow (measured 1-2 % on config 4)
+    if (w == 1) score *= 0.97;  // a single wave cannot rebalance CTAs that run slow
     if (score > best + 1e-9) { best = score; best_seg = seg; }
   }
   return best_seg;
