@@ -238,7 +238,7 @@ def run_ours(args, rank, world):
         droplets = {"B_th": args.droplets, "n_droplets": k, "ms": dms, "lb_steps": dms / step_ms,
                     "sites_min": float(st[:min(k, cap), 1].min()) if k else None,
                     "sites_max": float(st[:min(k, cap), 1].max()) if k else None,
-                    "call": "tlb_droplets (fields pass for rho_A, threshold, union-find labelling, flatten, statistics)"}
+                    "call": "tlb_droplets (rho_A from the first fluid's 9 planes, threshold + run labels, union-find on the remaining bonds, flatten, statistics)"}
         # second stage (R23-R26): digital Voronoi colouring of the centres, Delaunay links, droplet Nusselt numbers
         kk = min(k, cap)
         if kk > 0:

@@ -252,24 +252,87 @@ __global__ void t1_rank_kernel(const int* __restrict__ tmp, const int* __restric
   if (rank < max_events) { events[4 * rank] = e0; events[4 * rank + 1] = e1; events[4 * rank + 2] = e2; events[4 * rank + 3] = e3; }
 }
 
-// ---- R26: droplet Nusselt number, Eq. (25), from the fields u_y^(H) and T at the site nearest to the centre
-__global__ void droplet_nusselt_kernel(const Dev d, const double* __restrict__ uy, const double* __restrict__ T,
-                                       const double* __restrict__ centres, int n, double tau_g, double* __restrict__ nu) {
+// ---- R26: droplet Nusselt number, Eq. (25).  The fields are needed at one site per droplet only, so they are evaluated
+// there directly from the pull-form buffer (Eqs. (4)-(12), (17), (22), L139 written out for one site) instead of
+// sweeping the lattice: a few hundred loads per droplet.
+__device__ __forceinline__ double w_of(int c2) { return c2 == 1 ? 1.0 / 9.0 : (c2 == 2 ? 1.0 / 36.0 : 0.0); }
+__device__ __forceinline__ double p_of(int c2) {
+  return c2 == 1 ? 4.0 / 63.0 : c2 == 2 ? 4.0 / 135.0 : c2 == 4 ? 1.0 / 180.0 : c2 == 5 ? 2.0 / 945.0 : c2 == 8 ? 1.0 / 15120.0 : 0.0;
+}
+__device__ __forceinline__ int wrapc(int a, int n) { return a < 0 ? a + n : (a >= n ? a - n : a); }
+
+// is node (x, y) solid (a wall row beyond the lattice counts); x any column within 4 of the lattice, y any row
+__device__ __forceinline__ bool solid_at(const Dev& d, int x, int& y) {
+  if (d.periodic_y) y = wrapc(y, d.ny);
+  else if (y < 0 || y >= d.ny) return true;
+  return d.solid[(size_t)y * d.nx + wrapc(x, d.nx)] != 0;
+}
+// sum over i of S_set,i(n - c_i) at a fluid node n = (x, y) (y in range): a density (set 0, 1) or the temperature (set 2)
+template <typename ST>
+__device__ __forceinline__ double moment0(const Dev& d, const ST* __restrict__ S, int set, int x, int y) {
+  double a = 0.0;
+#pragma unroll
+  for (int i = 0; i < 9; i++) {
+    int sy = y - cy(i);
+    if (d.periodic_y) sy = wrapc(sy, d.ny);
+    a += (double)S[(9 * set + pslot(i)) * d.plane + d.at(x - cx(i), sy)];
+  }
+  return a;
+}
+
+template <typename ST>
+__global__ void droplet_nusselt_kernel(const Dev d, const ST* __restrict__ S, const double* __restrict__ centres, int n,
+                                       double tau_g, double* __restrict__ nu) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int nx = d.nx, ny = d.ny;
   const bool per = d.periodic_y != 0;
   const int x = nearest_site(centres[2 * i], nx, true), y = nearest_site(centres[2 * i + 1], ny, per);
-  const size_t k = (size_t)y * nx + x;
   const double DT = d.T_bottom - d.T_top;
-  if (d.solid[k] || DT == 0.0) { nu[i] = 0.0; return; }
+  if (d.solid[(size_t)y * nx + x] || DT == 0.0) { nu[i] = 0.0; return; }
+  // moments of the site
+  const double rA = moment0(d, S, 0, x, y), rB = moment0(d, S, 1, x, y), T = moment0(d, S, 2, x, y);
+  double jy = 0.0;
+#pragma unroll
+  for (int k = 0; k < 9; k++) {
+    if (cy(k) == 0) continue;
+    int sy = y - cy(k);
+    if (per) sy = wrapc(sy, ny);
+    const long long o = d.at(x - cx(k), sy);
+    jy += (double)cy(k) * ((double)S[pslot(k) * d.plane + o] + (double)S[(9 + pslot(k)) * d.plane + o]);
+  }
+  // y components of the interaction forces, Eqs. (7), (10), (11), wall values at solid nodes (L155)
+  const double psA = d.rho0 * (1.0 - exp(-rA * d.inv_rho0)), psB = d.rho0 * (1.0 - exp(-rB * d.inv_rho0));
+  double XA = 0.0, XB = 0.0, SA = 0.0, SB = 0.0;
+  for (int dy = -2; dy <= 2; dy++)
+    for (int dx = -2; dx <= 2; dx++) {
+      const int c2 = dx * dx + dy * dy;
+      if (c2 == 0 || dy == 0) continue;
+      int yy = y + dy;
+      double a, b, pa, pb;
+      if (solid_at(d, x + dx, yy)) {
+        a = d.rho_wall_A; b = d.rho_wall_B; pa = d.pss_wall_A; pb = d.pss_wall_B;
+      } else {
+        a = moment0(d, S, 0, x + dx, yy); b = moment0(d, S, 1, x + dx, yy);
+        pa = d.rho0 * (1.0 - exp(-a * d.inv_rho0)); pb = d.rho0 * (1.0 - exp(-b * d.inv_rho0));
+      }
+      XA += w_of(c2) * dy * b;  // cross force on A sees psi^x of B, and the other way round
+      XB += w_of(c2) * dy * a;
+      SA += (d.G11a * w_of(c2) + d.G11r * p_of(c2)) * dy * pa;
+      SB += (d.G22a * w_of(c2) + d.G22r * p_of(c2)) * dy * pb;
+    }
+  const double gx = d.G12 * d.inv_rho0 * d.inv_rho0;
+  const double dTb = d.thermal ? (T - d.T_ref) : 0.0;
+  const double FAy = -gx * rA * XA - psA * SA + rA * d.alpha_g * dTb;
+  const double FBy = -gx * rB * XB - psB * SB + rB * d.alpha_g * dTb;
+  const double uy = (jy + 0.5 * (FAy + FBy)) / (rA + rB);  // L139
+  // d_y T as in Eq. (24) / R10
   int yu = y + 1, yd = y - 1;
-  if (per) { yu = yu >= ny ? 0 : yu; yd = yd < 0 ? ny - 1 : yd; }
-  const bool su = yu >= ny || d.solid[(size_t)yu * nx + x], sd = yd < 0 || d.solid[(size_t)yd * nx + x];
-  const double up = su ? d.T_wall(yu) : 0.5 * (T[k] + T[(size_t)yu * nx + x]);
-  const double dn = sd ? d.T_wall(yd) : 0.5 * (T[k] + T[(size_t)yd * nx + x]);
+  const bool su = solid_at(d, x, yu), sd = solid_at(d, x, yd);
+  const double up = su ? d.T_wall(y + 1) : 0.5 * (T + moment0(d, S, 2, x, yu));
+  const double dn = sd ? d.T_wall(y - 1) : 0.5 * (T + moment0(d, S, 2, x, yd));
   const double kappa = (tau_g - 0.5) / 3.0;
-  nu[i] = (uy[k] * T[k] - kappa * (up - dn)) / (kappa * DT / ny);
+  nu[i] = (uy * T - kappa * (up - dn)) / (kappa * DT / ny);
 }
 
 unsigned blocks_of(long long n, int t) { return (unsigned)((n + t - 1) / t); }
@@ -347,10 +410,10 @@ int launch_t1(const int* past, int n_past, const int* now, int n_now, const int*
   return launches + 1;
 }
 
-int launch_droplet_nusselt(const Dev& d, const double* uy, const double* T, const double* centres, int n, double tau_g,
-                           double* nu, cudaStream_t st) {
+int launch_droplet_nusselt(const Dev& d, const void* S, const double* centres, int n, double tau_g, double* nu, cudaStream_t st) {
   if (n <= 0) return 0;
-  droplet_nusselt_kernel<<<blocks_of(n, 128), 128, 0, st>>>(d, uy, T, centres, n, tau_g, nu);
+  if (d.prec == 32) droplet_nusselt_kernel<float><<<blocks_of(n, 64), 64, 0, st>>>(d, static_cast<const float*>(S), centres, n, tau_g, nu);
+  else droplet_nusselt_kernel<double><<<blocks_of(n, 64), 64, 0, st>>>(d, static_cast<const double*>(S), centres, n, tau_g, nu);
   return 1;
 }
 

@@ -924,10 +924,7 @@ int tlb_droplets(tlb_handle* h, double B_th, int32_t* labels, int32_t max_drople
   if ((size_t)max_droplets * 4 > n) return TLB_EINVAL;  // root lists and sums live in scratch planes
   if (!h->has_state) return TLB_ESTATE;
   TLB_ENTER(h);
-  FusedOut o{};
-  o.rhoA = h->fld[0];
-  int rc = fused_mode(h, 1, o);
-  if (rc != TLB_OK) return rc;
+  h->launches += launch_rho_a(h->d, h->S[h->cur], h->fld[0], h->st);  // only the first fluid's 9 planes are read
   int* lab = labels ? labels : reinterpret_cast<int*>(h->fld[1]);
   h->launches += launch_label_init(h->d, h->fld[0], B_th, lab, h->st);
   h->launches += launch_label_merge(h->d, lab, h->st);
@@ -957,7 +954,7 @@ int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_d
 }
 
 // ---- droplet analysis, second stage (section 2.4, Eq. (25); readings R23-R26).  Scratch planes fld[2], fld[3]
-// hold the cell grid / adjacency tables / events found; fld[3], fld[4] the fields of the Nusselt call.
+// hold the cell grid / adjacency tables / events found.
 int tlb_voronoi(tlb_handle* h, const double* centres, int32_t n, int32_t* colour) {
   if (!h || !colour || n < 0 || (n > 0 && !centres)) return TLB_EINVAL;
   if (h->slab) return TLB_EINVAL;
@@ -1009,11 +1006,7 @@ int tlb_droplet_nusselt(tlb_handle* h, const double* centres, int32_t n, double*
   if (h->slab) return TLB_EINVAL;
   if (!h->has_state || h->step_open) return TLB_ESTATE;
   TLB_ENTER(h);
-  FusedOut o{};
-  o.uy = h->fld[3]; o.T = h->fld[4];
-  int rc = fused_mode(h, 1, o);
-  if (rc != TLB_OK) return rc;
-  h->launches += launch_droplet_nusselt(h->d, h->fld[3], h->fld[4], centres, n, h->p.tau_g, nu, h->st);
+  h->launches += launch_droplet_nusselt(h->d, h->S[h->cur], centres, n, h->p.tau_g, nu, h->st);
   return check(h);
 }
 

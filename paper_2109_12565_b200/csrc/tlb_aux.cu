@@ -274,10 +274,35 @@ __global__ void halo_copy_kernel(const Dev d, ST* __restrict__ S, int face, ST* 
 // nearest-neighbour (4-connected) bulk sites, x periodic (y too when the lattice is), label = smallest site index
 // y nx + x of the cluster.  Lock-free union-find: every union hangs the larger root under the smaller one with
 // atomicMin, so parents only decrease and the root of a finished cluster is its smallest index.
+// One warp = 32 consecutive sites of one row.  A bulk site starts as a child of the leftmost site of its run of bulk
+// sites inside the warp's window (a parent with a smaller index, like every parent later on): the horizontal bonds inside
+// a window need no union at all.
 __global__ void label_init_kernel(const Dev d, const double* __restrict__ rhoA, double threshold, int* __restrict__ labels) {
-  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (q >= (size_t)d.nx * d.ny) return;
-  labels[q] = (!d.solid[q] && rhoA[q] > threshold) ? (int)q : -1;
+  const int x = blockIdx.y * blockDim.x + threadIdx.x, y = blockIdx.x;  // rows on grid.x (no 65535 limit)
+  const size_t q = (size_t)y * d.nx + (x < d.nx ? x : 0);
+  const bool bulk = x < d.nx && !d.solid[q] && rhoA[q] > threshold;
+  const unsigned m = __ballot_sync(0xffffffffu, bulk);
+  if (x >= d.nx) return;
+  const int lane = threadIdx.x & 31;
+  const unsigned holes_below = ~m & ((1u << lane) - 1u);           // non-bulk lanes to the left of this one
+  const int start = holes_below ? 32 - __clz(holes_below) : 0;     // first lane of this lane's run
+  labels[q] = bulk ? (int)q - (lane - start) : -1;
+}
+
+// rho_A = sum_i f_A,i (Eq. (4)) of the current state for the threshold: the 9 planes of the first fluid only, pulled
+// from the pull-form buffer (ghost rows and columns hold what a fluid site pulls), same summation order as the fused kernel
+template <typename ST>
+__global__ void rho_a_kernel(const Dev d, const ST* __restrict__ S, double* __restrict__ rhoA) {
+  const int x = blockIdx.y * blockDim.x + threadIdx.x, y = blockIdx.x;  // rows on grid.x (no 65535 limit)
+  if (x >= d.nx) return;
+  double f[9];
+#pragma unroll
+  for (int i = 0; i < 9; i++) {
+    int sy = y - cy(i);
+    if (d.periodic_y) sy = wrapi(sy, d.ny);
+    f[i] = (double)S[pslot(i) * d.plane + d.at(x - cx(i), sy)];
+  }
+  rhoA[(size_t)y * d.nx + x] = (((f[0] + f[1]) + (f[2] + f[3])) + ((f[4] + f[5]) + (f[6] + f[7]))) + f[8];
 }
 
 __device__ __forceinline__ int find_root(volatile int* L, int i) {
@@ -312,21 +337,23 @@ __device__ __forceinline__ void unite(int* L, int a, int b) {
   } while (!done);
 }
 
+// Bonds that still need a union: the horizontal bond into a warp window (its first lane and the site to its left, which
+// for x = 0 is the periodic image x = nx - 1), and of the vertical bonds between two rows only the leftmost one of every
+// stretch where both rows are bulk -- the bonds to its right connect the same two runs again.  (x = 0 never defers to
+// its periodic left neighbour: two completely bulk rows would otherwise wait for one another all around the ring.)
 __global__ void label_merge_kernel(const Dev d, int* __restrict__ labels) {
-  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (q >= (size_t)d.nx * d.ny) return;
+  const int x = blockIdx.y * blockDim.x + threadIdx.x, y = blockIdx.x;  // rows on grid.x (no 65535 limit)
+  if (x >= d.nx) return;
+  const size_t q = (size_t)y * d.nx + x;
   if (labels[q] < 0) return;
-  const int x = (int)(q % d.nx), y = (int)(q / d.nx);
-  const int xr = x + 1 < d.nx ? x + 1 : 0;
-  if (xr != x) {  // bond to the right-hand neighbour (periodic in x, L147)
-    const int n = y * d.nx + xr;
-    if (labels[n] >= 0) unite(labels, (int)q, n);
-  }
+  const int xl = x > 0 ? x - 1 : d.nx - 1;
+  const bool left = xl != x && labels[(size_t)y * d.nx + xl] >= 0;
+  if (left && ((threadIdx.x & 31) == 0)) unite(labels, (int)q, y * d.nx + xl);  // x = 0 is lane 0 of its warp
   int yu = y + 1;
   if (yu >= d.ny) yu = d.periodic_y ? 0 : -1;
-  if (yu >= 0 && yu != y) {  // bond to the neighbour above
-    const int n = yu * d.nx + x;
-    if (labels[n] >= 0) unite(labels, (int)q, n);
+  if (yu >= 0 && yu != y && labels[(size_t)yu * d.nx + x] >= 0) {
+    const bool left_pair = x > 0 && left && labels[(size_t)yu * d.nx + xl] >= 0;
+    if (!left_pair) unite(labels, (int)q, yu * d.nx + x);
   }
 }
 
@@ -372,13 +399,22 @@ __device__ __forceinline__ int min_image(int a, int b, int n) {
   return dlt;
 }
 
-// per droplet: sites, sum of x offsets and of y offsets from the root site -- integer atomics, order-independent
+// per droplet: sites, sum of x offsets and of y offsets from the root site -- integer atomics, order-independent.
+// The lanes of a warp (32 consecutive sites of a row) that belong to the same droplet add up first: one search and
+// three atomics per group instead of per site.
 __global__ void droplet_sums_kernel(const Dev d, const int* __restrict__ labels, const int* __restrict__ sorted,
                                     int max_droplets, const int* __restrict__ n_out, unsigned long long* __restrict__ sums) {
-  const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (q >= (size_t)d.nx * d.ny) return;
-  const int root = labels[q];
-  if (root < 0) return;
+  const int x = blockIdx.y * blockDim.x + threadIdx.x, y = blockIdx.x;  // rows on grid.x (no 65535 limit)
+  const int root = x < d.nx ? labels[(size_t)y * d.nx + x] : -1;
+  const unsigned peers = __match_any_sync(0xffffffffu, root);
+  int dx = 0, dy = 0;
+  if (root >= 0) {
+    const int xr = root % d.nx, yr = root / d.nx;
+    dx = min_image(x, xr, d.nx);
+    dy = d.periodic_y ? min_image(y, yr, d.ny) : y - yr;
+  }
+  const int sdx = __reduce_add_sync(peers, dx), sdy = __reduce_add_sync(peers, dy);
+  if (root < 0 || (int)(threadIdx.x & 31) != __ffs(peers) - 1) return;  // the lowest lane of the group goes on
   const int n = min(*n_out, max_droplets);
   int lo = 0, hi = n;  // lower bound of root in sorted[0, n)
   while (lo < hi) {
@@ -387,12 +423,9 @@ __global__ void droplet_sums_kernel(const Dev d, const int* __restrict__ labels,
     else hi = mid;
   }
   if (lo >= n || sorted[lo] != root) return;  // a droplet beyond max_droplets
-  const int x = (int)(q % d.nx), y = (int)(q / d.nx), xr = root % d.nx, yr = root / d.nx;
-  const long long dx = min_image(x, xr, d.nx);
-  const long long dy = d.periodic_y ? min_image(y, yr, d.ny) : y - yr;
-  atomicAdd(&sums[3 * lo + 0], 1ull);
-  atomicAdd(&sums[3 * lo + 1], (unsigned long long)dx);  // two's complement: wraps to the signed sum
-  atomicAdd(&sums[3 * lo + 2], (unsigned long long)dy);
+  atomicAdd(&sums[3 * lo + 0], (unsigned long long)__popc(peers));
+  atomicAdd(&sums[3 * lo + 1], (unsigned long long)(long long)sdx);  // two's complement: wraps to the signed sum
+  atomicAdd(&sums[3 * lo + 2], (unsigned long long)(long long)sdy);
 }
 
 // stats[k] = {label, sites, centre x, centre y} in ascending label order; centre = root + mean offset, wrapped
@@ -493,12 +526,18 @@ int launch_perturb(const Dev& d, double amplitude, double* fA, double* fB, cudaS
   perturb_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, amplitude, fA, fB);
   return 1;
 }
+int launch_rho_a(const Dev& d, const void* S, double* rhoA, cudaStream_t st) {
+  const dim3 g(d.ny, blocks_for(d.nx, 256));
+  if (d.prec == 32) rho_a_kernel<float><<<g, 256, 0, st>>>(d, static_cast<const float*>(S), rhoA);
+  else rho_a_kernel<double><<<g, 256, 0, st>>>(d, static_cast<const double*>(S), rhoA);
+  return 1;
+}
 int launch_label_init(const Dev& d, const double* rhoA, double threshold, int* labels, cudaStream_t st) {
-  label_init_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, rhoA, threshold, labels);
+  label_init_kernel<<<dim3(d.ny, blocks_for(d.nx, 256)), 256, 0, st>>>(d, rhoA, threshold, labels);
   return 1;
 }
 int launch_label_merge(const Dev& d, int* labels, cudaStream_t st) {
-  label_merge_kernel<<<blocks_for((long long)d.nx * d.ny, 256), 256, 0, st>>>(d, labels);
+  label_merge_kernel<<<dim3(d.ny, blocks_for(d.nx, 256)), 256, 0, st>>>(d, labels);
   return 1;
 }
 int launch_label_flatten(const Dev& d, int* labels, cudaStream_t st) {
@@ -512,7 +551,7 @@ int launch_droplet_stats(const Dev& d, const int* labels, int* roots, int* sorte
   const unsigned nb = blocks_for((long long)d.nx * d.ny, 256);
   droplet_roots_kernel<<<nb, 256, 0, st>>>(d, labels, roots, max_droplets, n_out);
   droplet_rank_kernel<<<blocks_for(max_droplets, 256), 256, 0, st>>>(roots, max_droplets, n_out, sorted);
-  droplet_sums_kernel<<<nb, 256, 0, st>>>(d, labels, sorted, max_droplets, n_out, sums);
+  droplet_sums_kernel<<<dim3(d.ny, blocks_for(d.nx, 256)), 256, 0, st>>>(d, labels, sorted, max_droplets, n_out, sums);
   droplet_finish_kernel<<<blocks_for(max_droplets, 256), 256, 0, st>>>(d, sorted, sums, max_droplets, n_out, stats);
   return 4;
 }

@@ -124,6 +124,7 @@ int launch_observables_from_sums(const Dev& d, const double* sums6, double* out4
 int launch_x_average(const Dev& d, const double* plane, double* av, cudaStream_t st);
 int launch_halo_pack(const Dev& d, const void* S, int face, void* buf, cudaStream_t st);
 int launch_halo_unpack(const Dev& d, void* S, int face, const void* buf, cudaStream_t st);
+int launch_rho_a(const Dev& d, const void* S, double* rhoA, cudaStream_t st);
 int launch_label_init(const Dev& d, const double* rhoA, double threshold, int* labels, cudaStream_t st);
 int launch_label_merge(const Dev& d, int* labels, cudaStream_t st);
 int launch_label_flatten(const Dev& d, int* labels, cudaStream_t st);
@@ -142,8 +143,7 @@ int launch_delaunay(const Dev& d, const int* colour, int n, int* scratch, int ma
 int launch_match(const Dev& d, const int* colour_past, const double* centres_now, int n_now, int* map, cudaStream_t st);
 int launch_t1(const int* past, int n_past, const int* now, int n_now, const int* map, int n_map, int n, int* scratch, int cap,
               int max_events, int* n_events, int* events, cudaStream_t st);
-int launch_droplet_nusselt(const Dev& d, const double* uy, const double* T, const double* centres, int n, double tau_g,
-                           double* nu, cudaStream_t st);
+int launch_droplet_nusselt(const Dev& d, const void* S, const double* centres, int n, double tau_g, double* nu, cudaStream_t st);
 int launch_rough_walls(const Dev& d, const int* cut, int height, int up, int down, int width, int lambda, int asymmetric,
                        uint8_t* solid, cudaStream_t st);
 int launch_perturb(const Dev& d, double amplitude, double* fA, double* fB, cudaStream_t st);

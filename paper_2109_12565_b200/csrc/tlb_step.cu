@@ -19,8 +19,10 @@
 // planes are only needed in (2) and go straight to registers (LDG issued before the row barrier).
 // The eight warps of a CTA never meet at a CTA-wide barrier: each warp keeps its own rho / psi ring
 // for its 16 columns plus a 2-cell halo (the 4 halo columns are recomputed, not exchanged), waits
-// on the mbarrier of the row it needs, and counts itself out of the slot it has finished with; the
-// last warp out issues the copy of row r+2 into that slot, a full row of compute ahead of its use.
+// on the "full" mbarrier of the row it needs and arrives on the "empty" mbarrier of the slot it has
+// finished with; the warps take turns re-arming the slots, each at the top of an iteration and with a
+// slot that the others left an iteration earlier, so that the issuing warp does not wait.
+// tau = 1 (the paper's Table A.3, every BASELINE config) has its own instantiation: see Smem.
 #include "tlb_internal.cuh"
 
 namespace tlb {
