@@ -202,6 +202,14 @@ int tlb_slab_step_interior(tlb_handle* h);
 int tlb_slab_step_finish(tlb_handle* h);
 int tlb_halo_pack(tlb_handle* h, int face, void* buf);
 int tlb_halo_unpack(tlb_handle* h, int face, const void* buf);
+/* Zero-copy alternative to pack / unpack: the population buffers keep the 27 plane rows of a lattice row next to one
+ * another, so the 3 rows on either side of a face are ONE contiguous block of tlb_halo_bytes.  which = 0: the owned rows
+ * next to `face` (what the neighbour imports); which = 1: the halo rows beyond `face` (where the neighbour's rows go).
+ * *ptr is a DEVICE pointer into the buffer pack / unpack would address at this moment (the one being written while a
+ * step is open); it changes from step to step (double buffer).  A transport (NCCL send / recv, a peer-to-peer copy, a
+ * kernel of the neighbour storing through a peer mapping) can read the first and write the second directly, ordered
+ * after tlb_slab_step_edges and before tlb_slab_step_finish on the handle's stream.  Same error codes as tlb_halo_pack. */
+int tlb_halo_region(tlb_handle* h, int face, int which, void** ptr, size_t* bytes);
 
 /* Measurement aid: advance ONE step, launching the fused kernel n (1..4096) times back to back on the
  * same input / output buffers and then the boundary kernel n times (both are idempotent on fixed inputs),

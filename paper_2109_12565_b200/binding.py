@@ -25,6 +25,7 @@ SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destr
            "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
            "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step",
            "tlb_slab_step_edges", "tlb_slab_step_interior", "tlb_slab_step_finish", "tlb_halo_pack", "tlb_halo_unpack",
+           "tlb_halo_region",
            "tlb_profile_step", "tlb_fields", "tlb_fields_host", "tlb_observables", "tlb_observables_host",
            "tlb_observable_sums", "tlb_observables_from_sums", "tlb_x_average", "tlb_x_average_host",
            "tlb_stress_xy", "tlb_stress_xy_host", "tlb_x_average_stress", "tlb_x_average_stress_host",
@@ -119,6 +120,7 @@ def load_library():
     lib.tlb_seg_rows.argtypes = [vp]
     for name in ("tlb_slab_step_edges", "tlb_slab_step_interior", "tlb_slab_step_finish"):
         getattr(lib, name).argtypes = [vp]
+    lib.tlb_halo_region.argtypes = [vp, i32, i32, ctypes.POINTER(ctypes.c_void_p), ctypes.POINTER(ctypes.c_size_t)]
     lib.tlb_halo_pack.argtypes = [vp, i32, dp]
     lib.tlb_halo_unpack.argtypes = [vp, i32, dp]
     lib.tlb_droplets.argtypes = [vp, ctypes.c_double, dp, i32, dp, dp]
@@ -466,6 +468,15 @@ class TLB:
 
     def slab_step_finish(self):
         self._chk(self.lib.tlb_slab_step_finish(self.h))
+
+    def halo_region(self, face, which):
+        """uint8 view (no copy) of the 3 owned rows next to `face` (which = 0) or of the halo rows beyond it (which = 1) in
+        the population buffer that tlb_halo_pack / _unpack would address now."""
+        p, nb = ctypes.c_void_p(), ctypes.c_size_t()
+        self._chk(self.lib.tlb_halo_region(self.h, int(face), int(which), ctypes.byref(p), ctypes.byref(nb)))
+        off = p.value - self.workspace.data_ptr()
+        assert 0 <= off and off + nb.value <= self.workspace.numel()
+        return self.workspace[off:off + nb.value]
 
     def halo_pack(self, face, buf):
         self._chk(self.lib.tlb_halo_pack(self.h, int(face), buf.data_ptr()))

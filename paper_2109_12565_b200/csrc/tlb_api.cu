@@ -748,6 +748,20 @@ int tlb_halo_unpack(tlb_handle* h, int face, const void* buf) {
   return check(h);
 }
 
+int tlb_halo_region(tlb_handle* h, int face, int which, void** ptr, size_t* bytes) {
+  if (!h || !ptr || !bytes || face < 0 || face > 1 || which < 0 || which > 1 || !(face ? h->halo_hi : h->halo_lo)) return TLB_EINVAL;
+  if (!h->has_state) return TLB_ESTATE;
+  const Dev& d = h->d;
+  const size_t esz = d.prec == 32 ? sizeof(float) : sizeof(double);
+  int y;  // first local row of the block
+  if (which == 0) y = face == 0 ? d.own0 : d.own1 - kHalo;
+  else y = face == 0 ? d.own0 - kHalo : d.own1;
+  char* S = static_cast<char*>(h->S[h->step_open ? 1 - h->cur : h->cur]);
+  *ptr = S + (size_t)(y + 1) * (size_t)d.row * esz;  // storage row y + 1; a row holds the 27 plane rows
+  *bytes = (size_t)kHalo * (size_t)d.row * esz;
+  return TLB_OK;
+}
+
 int tlb_profile_step(tlb_handle* h, int64_t n, double* fused_ms, double* boundary_ms) {
   if (!h || n < 1 || n > 4096 || !fused_ms || !boundary_ms) return TLB_EINVAL;
   if (h->halo_lo || h->halo_hi) return TLB_EINVAL;

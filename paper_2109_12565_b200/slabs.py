@@ -1,10 +1,12 @@
 """Y-slab multi-GPU driver (host logic only; every lattice operation is a call of the C ABI, include/tlb.h "Y-SLABS").
 
 One process per GPU owns a contiguous slab of rows of the nx x ny lattice (x stays periodic locally, the flat walls
-live on the first / last slab).  Per time step and interior face, the 3 owned rows next to the face (all 27 planes,
-packed by tlb_halo_pack) travel to the neighbour's halo rows: `torch.distributed` point-to-point (NCCL over NVLink
-on GPUs, gloo in the CPU tests of the host logic) on a side stream, overlapped with the fused kernel on the
-interior rows.  Observables are six partial sums per slab, all-reduced and finished by tlb_observables_from_sums.
+live on the first / last slab).  Per time step and interior face, the 3 owned rows next to the face (all 27 planes)
+travel to the neighbour's halo rows: `torch.distributed` point-to-point (NCCL over NVLink on GPUs, gloo in the CPU
+tests of the host logic) on a side stream, overlapped with the fused kernel on the interior rows.  The population
+buffers keep the 27 plane rows of a lattice row together, so those 3 rows are one contiguous block on both sides:
+the transport reads the sender's state and writes the receiver's halo rows directly (tlb_halo_region, zero copy);
+tlb_halo_pack / _unpack into separate buffers remain as the staged alternative (`zero_copy=False`).  Observables are six partial sums per slab, all-reduced and finished by tlb_observables_from_sums.
 The multi-GPU path is the paper's stated future work.
 
 This module holds none of the method's arithmetic and never imports anything under oracle/.
@@ -124,17 +126,29 @@ class Slab:
         return a[..., self.t.own0:self.t.own1, :]
 
     # ---- one time step in two halves, the exchange in between ---------------------------------
+    zero_copy = True  # exchange straight out of / into the population buffers (tlb_halo_region)
+
+    def regions(self):
+        """(send, recv): per face the views of the rows to export and of the halo rows to fill, in the buffer this step writes."""
+        send = [self.t.halo_region(f, 0) if nb is not None else None for f, nb in enumerate((self.lo, self.hi))]
+        recv = [self.t.halo_region(f, 1) if nb is not None else None for f, nb in enumerate((self.lo, self.hi))]
+        return send, recv
+
     def begin_step(self):
         self.t.slab_step_edges()
-        for face in (0, 1):
-            if self.send[face] is not None:
-                self.t.halo_pack(face, self.send[face])
+        if self.zero_copy:
+            self.send, self.recv = self.regions()
+        else:
+            for face in (0, 1):
+                if self.send[face] is not None:
+                    self.t.halo_pack(face, self.send[face])
         self.t.slab_step_interior()
 
     def end_step(self):
-        for face in (0, 1):
-            if self.recv[face] is not None:
-                self.t.halo_unpack(face, self.recv[face])
+        if not self.zero_copy:
+            for face in (0, 1):
+                if self.recv[face] is not None:
+                    self.t.halo_unpack(face, self.recv[face])
         self.t.slab_step_finish()
 
 
@@ -170,9 +184,12 @@ class DistributedSlab(Slab):
         torch, main = self.torch, self.t.stream
         for _ in range(n):
             self.t.slab_step_edges()
-            for face in (0, 1):
-                if self.send[face] is not None:
-                    self.t.halo_pack(face, self.send[face])
+            if self.zero_copy:
+                self.send, self.recv = self.regions()
+            else:
+                for face in (0, 1):
+                    if self.send[face] is not None:
+                        self.t.halo_pack(face, self.send[face])
             self.packed.record(main)
             self.t.slab_step_interior()              # overlaps the exchange below
             with torch.cuda.stream(self.comm_stream):

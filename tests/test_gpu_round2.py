@@ -341,6 +341,40 @@ def test_config2_long_run_observables(tlbmod, physics):
         print("config2[%s] step %6d  Nu %.9f  mass_A %.12e  mass_B %.12e  E %.6e  max|uH| %.4e" % ((physics,) + row))
 
 
+def test_slabs_staged_and_zero_copy_exchange_agree(tlbmod):
+    """The two transports of the halo rows -- straight out of / into the population buffers (tlb_halo_region) and through
+    tlb_halo_pack / _unpack buffers -- give bit-identical states; the regions are the documented rows."""
+    from paper_2109_12565_b200 import slabs as S
+    nx, ny, world = 200, 46, 3
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4)
+    solid = inputs.post_mask(nx, ny, 4, 4, 16)
+    solid[ny // 2 - 2:ny // 2 + 3, 30:37] = 1
+    rA, rB, T = inputs.smooth_random_fields(nx, ny, 2, 0.5, -0.5)
+    runs = []
+    for zc in (True, False):
+        sl = [S.Slab(nx, ny, r, world, **par) for r in range(world)]
+        for s in sl:
+            s.zero_copy = zc
+            s.set_solid(solid)
+            s.set_fields(rA, rB, T)
+        S.step_local(sl, 7)
+        runs.append([[_np(p) for p in s.t.get_populations()] for s in sl])
+    for a, b in zip(*runs):
+        for p, q in zip(a, b):
+            assert np.array_equal(p, q)
+    # a region is 3 whole storage rows (27 planes x padded pitch) of the buffer; face without halo rows -> TLB_EINVAL
+    s = S.Slab(nx, ny, 1, world, **par)
+    s.set_fields(rA, rB, T)
+    nb = s.t.halo_buffer().numel()
+    for face in (0, 1):
+        for which in (0, 1):
+            assert s.t.halo_region(face, which).numel() == nb
+    lo_send, lo_recv = s.t.halo_region(0, 0), s.t.halo_region(0, 1)
+    assert lo_send.data_ptr() - lo_recv.data_ptr() == nb          # the halo rows lie right below the owned rows
+    with pytest.raises(tlbmod.TLBError):
+        S.Slab(nx, ny, 0, world, **par).t.halo_region(0, 0)       # face 0 of slab 0 is a wall (and no state yet)
+
+
 def test_distributed_slab_world1_nccl(tlbmod):
     """The per-rank driver of the multi-GPU path (slabs.DistributedSlab: side stream, events, torch.distributed) with
     the only process group one GPU allows: world_size 1, NCCL, 127.0.0.1.  A y-periodic lattice makes the single slab
