@@ -285,6 +285,8 @@ int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_d
  *   droplet has more than 32 links.  n = number of colours (droplets).
  * tlb_droplet_match (R25): map[i] = colour_past at the site nearest to the present centre i (floor(c + 1/2), x wrapped,
  *   y wrapped or clamped): the past droplet in whose Voronoi cell the present droplet lies.
+ * tlb_droplet_displacements (L326, L340: the "Lagrangian droplet displacement vector fields" of the deltaAnalysis output):
+ *   disp[i] = X_i(now) - X_map[i](past) [n_now][2], minimum image in x (in y with periodic_y); (0, 0) where map[i] < 0.
  * tlb_t1_events (R25, "the diagonal link between a and b is replaced by the link between c and d"): both link lists as
  *   tlb_delaunay writes them; map (or NULL = identity; n_map entries) rewrites the ends of the present links into
  *   indices of the past frame (links with an end mapped to < 0 or both ends on one droplet are dropped); n_droplets =
@@ -296,6 +298,8 @@ int tlb_droplets_host(tlb_handle* h, double B_th, int32_t* labels, int32_t max_d
 int tlb_voronoi(tlb_handle* h, const double* centres, int32_t n, int32_t* colour);
 int tlb_delaunay(tlb_handle* h, const int32_t* colour, int32_t n, int32_t max_links, int32_t* n_links, int32_t* links);
 int tlb_droplet_match(tlb_handle* h, const int32_t* colour_past, const double* centres_now, int32_t n_now, int32_t* map);
+int tlb_droplet_displacements(tlb_handle* h, const double* centres_past, const double* centres_now, const int32_t* map,
+                              int32_t n_now, double* disp);
 int tlb_t1_events(tlb_handle* h, const int32_t* links_past, int32_t n_past, const int32_t* links_now, int32_t n_now,
                   const int32_t* map, int32_t n_map, int32_t n_droplets, int32_t max_events, int32_t* n_events,
                   int32_t* events);

@@ -707,6 +707,24 @@ void orc_match(int nx, int ny, int periodic_y, const int32_t *colour_past, const
     map[i] = colour_past[(size_t)nearest_site(centres_now[2 * i + 1], ny, periodic_y) * nx + nearest_site(centres_now[2 * i], nx, 1)];
 }
 
+/* Droplet displacement field (L326, L340: "Lagrangian droplet displacement vector fields d(X_i(t), t) ... computed for all
+ * droplet centre-of-mass"; the deltaAnalysis output): d_i = X_i(now) - X_map[i](past), minimum image in x (and in y when
+ * periodic); a droplet without a past partner (map < 0) gets (0, 0). */
+void orc_displacements(int nx, int ny, int periodic_y, const double *centres_past, const double *centres_now, const int32_t *map,
+                       int n_now, double *disp) {
+  for (int i = 0; i < n_now; i++) {
+    double dx = 0.0, dy = 0.0;
+    if (map[i] >= 0) {
+      dx = centres_now[2 * i] - centres_past[2 * map[i]];
+      dy = centres_now[2 * i + 1] - centres_past[2 * map[i] + 1];
+      const double hx = 0.5 * (double)nx, hy = 0.5 * (double)ny;
+      if (dx > hx) dx -= (double)nx; else if (dx < -hx) dx += (double)nx;
+      if (periodic_y) { if (dy > hy) dy -= (double)ny; else if (dy < -hy) dy += (double)ny; }
+    }
+    disp[2 * i] = dx; disp[2 * i + 1] = dy;
+  }
+}
+
 static int has_pair(const int32_t *v, int n, int32_t a, int32_t b) {
   if (a > b) { const int32_t t = a; a = b; b = t; }
   for (int k = 0; k < n; k++)

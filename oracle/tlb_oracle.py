@@ -65,6 +65,7 @@ def _load():
         lib.orc_delaunay.restype = ctypes.c_int
         lib.orc_delaunay.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, ctypes.c_int, i32p]
         lib.orc_match.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, i32p, dp, ctypes.c_int, i32p]
+        lib.orc_displacements.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, i32p, ctypes.c_int, dp]
         lib.orc_t1_events.restype = ctypes.c_int
         lib.orc_t1_events.argtypes = [i32p, ctypes.c_int, i32p, ctypes.c_int, i32p, ctypes.c_int, i32p]
         lib.orc_droplet_nusselt.argtypes = [ctypes.c_void_p, dp, ctypes.c_int, dp]
@@ -267,6 +268,15 @@ def match(colour_past, periodic_y, centres_now):
     m = np.zeros(len(c), dtype=np.int32)
     _load().orc_match(nx, ny, int(bool(periodic_y)), colour_past.ctypes.data, _dp(c), len(c), m.ctypes.data)
     return m
+
+
+def displacements(nx, ny, periodic_y, centres_past, centres_now, map_now_to_past):
+    """d_i = X_i(now) - X_map[i](past) in minimum image, [n_now][2]; (0, 0) for unmatched droplets."""
+    cp, cn = _c(centres_past).reshape(-1, 2), _c(centres_now).reshape(-1, 2)
+    mp = _i32(map_now_to_past)
+    out = np.zeros((len(cn), 2))
+    _load().orc_displacements(int(nx), int(ny), int(bool(periodic_y)), _dp(cp), _dp(cn), mp.ctypes.data, len(cn), _dp(out))
+    return out
 
 
 def t1_events(links_past, links_now, map_now_to_past=None, max_events=4096):

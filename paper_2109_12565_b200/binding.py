@@ -29,7 +29,7 @@ SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destr
            "tlb_profile_step", "tlb_fields", "tlb_fields_host", "tlb_observables", "tlb_observables_host",
            "tlb_observable_sums", "tlb_observables_from_sums", "tlb_x_average", "tlb_x_average_host",
            "tlb_stress_xy", "tlb_stress_xy_host", "tlb_x_average_stress", "tlb_x_average_stress_host",
-           "tlb_droplets", "tlb_droplets_host", "tlb_voronoi", "tlb_delaunay", "tlb_droplet_match", "tlb_t1_events",
+           "tlb_droplets", "tlb_droplets_host", "tlb_voronoi", "tlb_delaunay", "tlb_droplet_match", "tlb_droplet_displacements", "tlb_t1_events",
            "tlb_droplet_nusselt", "tlb_launch_count", "tlb_error_string", "tlb_last_cuda_error"]
 
 
@@ -128,6 +128,7 @@ def load_library():
     lib.tlb_voronoi.argtypes = [vp, dp, i32, dp]
     lib.tlb_delaunay.argtypes = [vp, dp, i32, i32, dp, dp]
     lib.tlb_droplet_match.argtypes = [vp, dp, dp, i32, dp]
+    lib.tlb_droplet_displacements.argtypes = [vp, dp, dp, dp, i32, dp]
     lib.tlb_t1_events.argtypes = [vp, dp, i32, dp, i32, dp, i32, i32, i32, dp, dp]
     lib.tlb_droplet_nusselt.argtypes = [vp, dp, i32, dp]
     lib.tlb_launch_count.argtypes = [vp]
@@ -426,6 +427,15 @@ class TLB:
             self._chk(self.lib.tlb_droplet_match(self.h, colour_past.data_ptr(), _ptr(centres_now), int(centres_now.shape[0]),
                                                  m.data_ptr()))
             return m[:int(centres_now.shape[0])]
+
+    def droplet_displacements(self, centres_past, centres_now, map_now_to_past):
+        """d_i = X_i(now) - X_map[i](past) [n_now][2] in minimum image (device tensor)."""
+        with self.torch.cuda.stream(self.stream):
+            torch = self.torch
+            cp, cn, mp = centres_past.contiguous(), centres_now.contiguous(), map_now_to_past.contiguous()
+            out = torch.zeros((max(1, int(cn.shape[0])), 2), dtype=torch.float64, device=self.device)
+            self._chk(self.lib.tlb_droplet_displacements(self.h, _ptr(cp), _ptr(cn), _ptr(mp), int(cn.shape[0]), out.data_ptr()))
+            return out[:int(cn.shape[0])]
 
     def t1_events(self, links_past, links_now, n_droplets, map_now_to_past=None, max_events=4096):
         """(events [e][4] int32 = (a, b, c, d): link a-b replaced by c-d, n_events)."""

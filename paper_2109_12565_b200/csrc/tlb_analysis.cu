@@ -189,6 +189,24 @@ __global__ void match_kernel(const Dev d, const int* __restrict__ colour_past, c
   map[i] = colour_past[(size_t)nearest_site(centres[2 * i + 1], d.ny, d.periodic_y != 0) * d.nx + nearest_site(centres[2 * i], d.nx, true)];
 }
 
+// displacement of every present droplet from its past partner (minimum image), (0, 0) without one
+__global__ void displacement_kernel(const Dev d, const double* __restrict__ past, const double* __restrict__ now,
+                                    const int* __restrict__ map, int n, double* __restrict__ disp) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double dx = 0.0, dy = 0.0;
+  const int m = map[i];
+  if (m >= 0) {
+    dx = __dsub_rn(now[2 * i], past[2 * m]);
+    dy = __dsub_rn(now[2 * i + 1], past[2 * m + 1]);
+    const double hx = 0.5 * (double)d.nx, hy = 0.5 * (double)d.ny;
+    if (dx > hx) dx -= (double)d.nx; else if (dx < -hx) dx += (double)d.nx;
+    if (d.periodic_y) { if (dy > hy) dy -= (double)d.ny; else if (dy < -hy) dy += (double)d.ny; }
+  }
+  disp[2 * i] = dx;
+  disp[2 * i + 1] = dy;
+}
+
 // symmetric adjacency table of a link list; `map` (nullable) rewrites the ends, links with an end < 0, beyond n or
 // with equal ends are dropped
 __global__ void adj_build_kernel(const int* __restrict__ links, int n_links, const int* __restrict__ map, int n_map, int n,
@@ -383,6 +401,12 @@ int launch_delaunay(const Dev& d, const int* colour, int n, int* scratch, int ma
   scan_kernel<<<1, 1024, 0, st>>>(deg, n);
   del_write_kernel<<<blocks_of(n, 256), 256, 0, st>>>(adj, deg, n, max_links, overflow, n_links, links);
   return 4;
+}
+
+int launch_displacements(const Dev& d, const double* past, const double* now, const int* map, int n, double* disp, cudaStream_t st) {
+  if (n <= 0) return 0;
+  displacement_kernel<<<blocks_of(n, 256), 256, 0, st>>>(d, past, now, map, n, disp);
+  return 1;
 }
 
 int launch_match(const Dev& d, const int* colour_past, const double* centres_now, int n_now, int* map, cudaStream_t st) {

@@ -997,6 +997,15 @@ int tlb_droplet_match(tlb_handle* h, const int32_t* colour_past, const double* c
   return check(h);
 }
 
+int tlb_droplet_displacements(tlb_handle* h, const double* centres_past, const double* centres_now, const int32_t* map,
+                              int32_t n_now, double* disp) {
+  if (!h || n_now < 0 || (n_now > 0 && (!centres_past || !centres_now || !map || !disp))) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
+  TLB_ENTER(h);
+  h->launches += launch_displacements(h->d, centres_past, centres_now, map, n_now, disp, h->st);
+  return check(h);
+}
+
 int tlb_t1_events(tlb_handle* h, const int32_t* links_past, int32_t n_past, const int32_t* links_now, int32_t n_now,
                   const int32_t* map, int32_t n_map, int32_t n_droplets, int32_t max_events, int32_t* n_events,
                   int32_t* events) {

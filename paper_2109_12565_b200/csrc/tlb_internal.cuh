@@ -141,6 +141,7 @@ int launch_voronoi(const Dev& d, const double* centres, int n, int* scratch, int
 int launch_delaunay(const Dev& d, const int* colour, int n, int* scratch, int max_links, int* n_links, int* links,
                     cudaStream_t st);
 int launch_match(const Dev& d, const int* colour_past, const double* centres_now, int n_now, int* map, cudaStream_t st);
+int launch_displacements(const Dev& d, const double* past, const double* now, const int* map, int n, double* disp, cudaStream_t st);
 int launch_t1(const int* past, int n_past, const int* now, int n_now, const int* map, int n_map, int n, int* scratch, int cap,
               int max_events, int* n_events, int* events, cudaStream_t st);
 int launch_droplet_nusselt(const Dev& d, const void* S, const double* centres, int n, double tau_g, double* nu, cudaStream_t st);

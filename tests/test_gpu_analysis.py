@@ -159,6 +159,9 @@ def test_t1_events_between_two_frames(tlbmod, oracle_mod, per):
     assert (_np(lp) == olp).all() and (_np(ln) == oln).all()
     assert ne == one and (_np(ev) == oev).all()
     assert one >= (cols - 1) * (rows - 3)   # the interior squares all flip
+    disp = t.droplet_displacements(_dev(t, past, torch.float64), _dev(t, now, torch.float64), mp)
+    odisp = oracle_mod.displacements(nx, ny, per, past, now, omp)
+    assert (_np(disp) == odisp).all() and np.abs(odisp[:, 0]).max() > 1.0
     # truncation keeps the count and the sorted prefix
     ev2, ne2 = t.t1_events(lp, ln, len(past), mp, max_events=5)
     assert ne2 == one and (_np(ev2) == oev[:5]).all()

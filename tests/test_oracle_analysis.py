@@ -190,6 +190,18 @@ def test_match_follows_small_displacements(oracle_mod):
     assert (oracle_mod.match(col, 0, moved) == perm).all()
 
 
+def test_displacements_minimum_image(oracle_mod):
+    """d_i = X_i(now) - X_map[i](past): through the periodic seam in x always, in y only when periodic; (0, 0) unmatched."""
+    nx, ny = 100, 40
+    past = np.array([[98.0, 5.0], [10.0, 38.5], [50.0, 20.0]])
+    now = np.array([[50.5, 19.0], [1.5, 6.0], [12.0, 1.0], [70.0, 7.0]])
+    mp = np.array([2, 0, 1, -1], dtype=np.int32)
+    d = oracle_mod.displacements(nx, ny, 0, past, now, mp)
+    assert np.allclose(d, [[0.5, -1.0], [3.5, 1.0], [2.0, -37.5], [0.0, 0.0]], rtol=0, atol=1e-15)
+    d = oracle_mod.displacements(nx, ny, 1, past, now, mp)
+    assert np.allclose(d, [[0.5, -1.0], [3.5, 1.0], [2.0, 2.5], [0.0, 0.0]], rtol=0, atol=1e-15)
+
+
 def _grid_triangulation(cols, rows):
     """Links of a cols x rows grid of points, every square cut by its (i, j)-(i+1, j+1) diagonal."""
     idx = lambda i, j: j * cols + i
