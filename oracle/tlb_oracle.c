@@ -42,7 +42,8 @@
  *   perturbation       densities unchanged, momentum rho du, u^(H) = du on a rest state         L322 (R29)
  *   posts / corners    second, independently written streaming formulation
  *                      (orc_step_push_ghost) must agree bit for bit with the link-wise
- *                      pull of orc_step; beyond that and mass conservation the post-corner
+ *                      pull of orc_step, and the rule commutes with the symmetries of the lattice
+ *                      (transpose, mirrors); beyond that and mass conservation the post-corner
  *                      rule is a reading (R7/R19): "parity unpinned" for it.
  *
  * Build: gcc -O2 -ffp-contract=off -shared -fPIC -o liborc.so tlb_oracle.c -lm

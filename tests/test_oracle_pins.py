@@ -453,3 +453,46 @@ def test_x_average_with_posts_closed_form(oracle_mod):
     assert np.abs(got - expect).max() < 1e-15
     assert got[ny // 2] == 0.0
     assert np.abs(ux.mean(1) - expect)[:3].max() > 1e-4  # averaging over all nx sites would differ on post rows
+
+
+@pytest.mark.parametrize("sym", ["transpose", "mirror_x", "mirror_y"])
+def test_obstacle_rule_is_invariant_under_the_lattice_symmetries(oracle_mod, sym):
+    """The link-wise rule on obstacle faces and CORNERS (L151, R7/R19) has no closed form; what it must respect is the
+    symmetry group of the D2Q9 lattice.  A doubly periodic lattice with square and L-shaped obstacles (convex and concave
+    corners), full two-component physics and temperature, no gravity: the run on the transposed / mirrored geometry
+    and initial state is the transposed / mirrored run (up to the summation order of the stencils).  A corner rule that
+    prefers one axis or one sense of a diagonal fails this."""
+    n = 24
+    par = dict(PAPER_FORCES, tau=0.9, tau_g=1.2, rho_wall_A=0.5, rho_wall_B=0.7, T_bottom=0.3, T_top=0.3, periodic_y=1)
+    solid = np.zeros((n, n), np.uint8)
+    solid[5:9, 6:10] = 1                      # a square post in the bulk
+    solid[14:19, 12:14] = 1                   # an L: a concave corner at its elbow
+    solid[17:19, 14:18] = 1
+    rA, rB, T = inputs.smooth_random_fields(n, n, 41, 0.3, 0.3, 0.25)
+    T = 0.3 + 0.2 * (rA - rA.mean())
+    if sym == "transpose":
+        op = lambda a: np.swapaxes(a, -1, -2)
+        dmap = [0, 2, 1, 4, 3, 5, 8, 7, 6]    # direction with (c_x, c_y) swapped
+    elif sym == "mirror_x":
+        op = lambda a: a[..., ::-1]
+        dmap = [0, 3, 2, 1, 4, 6, 5, 8, 7]    # c_x -> -c_x
+    else:
+        op = lambda a: a[..., ::-1, :]
+        dmap = [0, 1, 4, 3, 2, 8, 7, 6, 5]    # c_y -> -c_y
+    cxy = [oracle_mod.directions()[i][:2] for i in range(9)]
+    for i, j in enumerate(dmap):              # the map really is the symmetry acting on the direction set
+        cx, cy = cxy[i]
+        want = (cy, cx) if sym == "transpose" else ((-cx, cy) if sym == "mirror_x" else (cx, -cy))
+        assert tuple(cxy[j]) == want
+    runs = []
+    for g in (lambda a: a, op):
+        o = oracle_mod.Oracle(n, n, **par)
+        o.set_solid(np.ascontiguousarray(g(solid)))
+        o.set_fields(np.ascontiguousarray(g(rA)), np.ascontiguousarray(g(rB)), np.ascontiguousarray(g(T)))
+        o.step(40)
+        runs.append(o.get_populations())
+    for a, b in zip(*runs):
+        moved = op(a)[dmap]                   # the original run, carried over by the symmetry
+        assert np.abs(moved - b).max() < 5e-14
+    fA = runs[0][0]
+    assert np.abs(fA[1] - fA[3]).max() > 1e-3  # the state is not trivially symmetric itself
