@@ -18,7 +18,7 @@ struct tlb_handle {
   cudaStream_t st;
   int device;         // CUDA device of the workspace; every entry point runs with it current
   void* S[2];         // population buffers (pull form), 27 planes each, double or float (pop_precision)
-  TMaps maps[2];      // tensor maps of S[0], S[1] (fp64 storage only)
+  TMaps maps[2];      // tensor maps of S[0], S[1]
   bool has_maps;
   double* stage;      // [27][ny][nx] doubles for the *_host population calls when the buffers are float
   double* fld[5];     // rho_A, rho_B, u_x, u_y, T scratch planes
@@ -178,18 +178,20 @@ bool make_maps(tlb_handle* h) {
   }
   const encode_tiled_fn encode = reinterpret_cast<encode_tiled_fn>(fn);
   const Dev& d = h->d;
-  const cuuint64_t B = sizeof(double);
+  const bool f32 = d.prec == 32;
+  const cuuint64_t B = f32 ? sizeof(float) : sizeof(double);
+  const CUtensorMapDataType dt = f32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
   const cuuint64_t row = (cuuint64_t)d.row * B, plane = (cuuint64_t)d.plane * B;
   const cuuint64_t dims[5] = {(cuuint64_t)d.px, (cuuint64_t)d.ny + 2, 3, 3, 2};
   const cuuint64_t strides[4] = {row, plane, 3 * plane + row, 9 * plane};  // bytes, dimensions 1..4
-  const cuuint32_t box[5] = {(cuuint32_t)kCopyW, 1, 3, 3, 2};
+  const cuuint32_t box[5] = {(cuuint32_t)(f32 ? kCopyW + 8 : kCopyW), 1, 3, 3, 2};  // = the slot row pitch of the fused kernel
   const cuuint32_t ones[5] = {1, 1, 1, 1, 1};
   for (int k = 0; k < 2; k++) {
     char* base = static_cast<char*>(h->S[k]);
-    if (encode(&h->maps[k].f, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 5, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+    if (encode(&h->maps[k].f, dt, 5, base, dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return false;
-    if (encode(&h->maps[k].g, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base + 18 * plane, dims, strides, box, ones,
+    if (encode(&h->maps[k].g, dt, 4, base + 18 * plane, dims, strides, box, ones,
                CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return false;
@@ -423,11 +425,8 @@ static int create_common(int nx, int ny_glob, int y0, int y1, bool slab, const t
     h->use_graph = false;
   }
   if (configure_kernels() != 0) { cudaGetLastError(); tlb_destroy(h); return TLB_ECUDA; }
-  h->has_maps = false;
-  if (d.prec == 64) {
-    if (!make_maps(h)) { tlb_destroy(h); return TLB_ECUDA; }  // no second code path: fail loudly
-    h->has_maps = true;
-  }
+  if (!make_maps(h)) { tlb_destroy(h); return TLB_ECUDA; }  // no second code path: fail loudly
+  h->has_maps = true;
   cu(h, cudaMemsetAsync(h->solid, 0, (size_t)nx * ny, h->st));
   cu(h, cudaMemsetAsync(h->count, 0, sizeof(int), h->st));
   h->launches += launch_build_links(h->d, h->sites, h->count, h->solidp, h->st);  // padded mask of the empty flag field

@@ -97,7 +97,8 @@ struct FusedOut {
   double* partials;                   // MODE 3: [CTAs][6] {mass_A, mass_B, sum |u|^2, sum u_y T, sum d_y T, fluid sites}
 };
 
-// Tensor maps of one fp64 population buffer (built by tlb_create with cuTensorMapEncodeTiled):
+// Tensor maps of one population buffer (built by tlb_create with cuTensorMapEncodeTiled; box width = the slot row pitch:
+// kCopyW doubles, or kCopyW + 8 floats):
 //   f: 5-D (x, row, plane-in-group 3, c_y group 3, species 2), strides (1, row, plane, 3 plane + row, 9 plane);
 //   g: 4-D, the same without the species dimension, based at plane 18.
 // Row coordinate r addresses, in group k (c_y = 1 - k), storage row r + k = (r + 1) - c_y.
@@ -106,7 +107,7 @@ struct TMaps {
 };
 
 // launchers (each returns the number of kernels it launched)
-// maps: the tensor maps of the buffer Sin (fp64 storage), or null (fp32 storage: 1-D bulk copies)
+// maps: the tensor maps of the buffer Sin
 int launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
                  const TMaps* maps, cudaStream_t st);
 int fused_grid_ctas(const Dev& d, int seg_rows, int rows);  // CTAs launch_fused uses for `rows` rows

@@ -6,7 +6,7 @@
 // ONE tensor-map copy (cp.async.bulk.tensor.5d, TMA; SASS UTMALDG) whose box holds the strip of all 18 fluid
 // planes, each already shifted in y by the pull rule f_i(x, r) = S_i(x - c_i) (the planes are stored in c_y
 // order so that the shift is a stride of the tensor map, tlb_internal.cuh), into a 4-slot ring in shared
-// memory, completing on an mbarrier; the x shift is applied when threads read the ring.  (fp32 storage and the
+// memory, completing on an mbarrier; the x shift is applied when threads read the ring.  (The
 // two wrap rows of a y-periodic lattice use 18 1-D bulk copies, SASS UBLKCP, instead.)  Each landed row is
 // used twice without touching HBM or L2 again:
 //   (1) when it lands: rho_A, rho_B (Eq. (4)) and psi^s (Eq. (12)) of row r for the strip plus its
@@ -211,7 +211,7 @@ template <int MODE, bool PERIODIC, typename ST, bool TAU1>
 __global__ void __launch_bounds__(kThreads, kCtasPerSM)
 fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int seg_rows, int ya, int yb,
              const FusedOut out, const __grid_constant__ TMaps tm) {
-  constexpr bool kTensor = sizeof(ST) == 8;  // fp64 storage: tensor-map copies; fp32 (bandwidth study): 1-D bulk copies
+  constexpr bool kTensor = true;  // tensor-map row copies (1-D bulk copies remain for the two wrap rows of a y-periodic lattice)
   double* __restrict__ const oRA = out.rhoA;
   double* __restrict__ const oRB = out.rhoB;
   double* __restrict__ const oUx = out.ux;
@@ -258,12 +258,14 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     }
     const int sl = slot_of(q);
     uint64_t* bar = &sm.full[sl];
-    mbar_expect_tx(bar, 18u * kCopyW * kB);
     if (kTensor && (!PERIODIC || (rr > 0 && rr < ny - 1))) {
-      // one copy: box 136 x 1 x 3 x 3 x 2 = the 18 fluid plane rows, each shifted by its c_y (tlb_internal.cuh)
+      // one copy: box kSW x 1 x 3 x 3 x 2 = the 18 fluid plane rows, each shifted by its c_y (tlb_internal.cuh); kSW is
+      // the row pitch of a slot (136 doubles; 144 floats: the padding columns are fetched too, they exist in the buffer)
+      mbar_expect_tx(bar, 18u * kSW * kB);
       tma_g2s_5d(&sm.f[sl][0][0], &tm.f, kXL + x0 - kHX, rr, 0, 0, 0, bar, pol);
       return;
     }
+    mbar_expect_tx(bar, 18u * kCopyW * kB);
     const long long o0 = d.at(x0 - kHX, rr), om = d.at(x0 - kHX, rm), op = d.at(x0 - kHX, rp);
 #pragma unroll
     for (int l = 0; l < 2; l++)
@@ -806,8 +808,8 @@ static void launch_mode(const Dev& d, const void* Sin, void* Sout, int seg_rows,
 int launch_fused(const Dev& d, int mode, const void* Sin, void* Sout, int seg_rows, int ya, int yb, const FusedOut& out,
                  const TMaps* maps, cudaStream_t st) {
   if (yb <= ya) return 0;
-  static const TMaps none{};  // fp32 storage never reads the maps
-  const TMaps& tm = maps ? *maps : none;
+  static const TMaps none{};
+  const TMaps& tm = maps ? *maps : none;  // every handle has maps (tlb_create fails without them)
   if (seg_rows > yb - ya) seg_rows = yb - ya;
   if (seg_rows < 1) seg_rows = 1;
   const bool f32 = d.prec == 32;
