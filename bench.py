@@ -162,7 +162,7 @@ def run_ours(args, rank, world):
     torch.cuda.set_device(local)
     dev = "cuda:%d" % local
     binding.load_library()  # raises if libtlb.so is missing
-    if world > 1:
+    if world > 1 or args.force_slabs:
         return run_slabs(args, rank, world, local)
     cfg = inputs.config(args.config)
     nx, ny = cfg["nx"], cfg["ny"]
@@ -420,7 +420,7 @@ def run_slabs(args, rank, world, local):
     e2e_mlups, _ = replicas.aggregate_mlups(own_sites, e2e_steps, e2e_ms, dev)
     e2e = {"value": e2e_mlups, "unit": "MLUPS", "h2d_bytes_per_step": int(replicas.sum_over_ranks(3 * 8 * nx * nyl, dev)),
            "d2h_bytes_per_step": 32 * world, "steps": e2e_steps,
-           "call": "per rank: tlb_set_fields_host + slab step (edges, pack, interior, NCCL exchange, unpack, finish) + "
+           "call": "per rank: tlb_set_fields_host + slab step (edges, interior, NCCL exchange straight out of / into the population buffers, finish) + "
                    "tlb_observable_sums, all-reduce, tlb_observables_from_sums"}
     if rank == 0:
         print(json.dumps({
@@ -452,6 +452,8 @@ def main():
                     help="B_th > 0: also time tlb_droplets (threshold B_th on rho_A) on the final state and report it in LB steps")
     ap.add_argument("--observe-every", type=int, default=0,
                     help="also run the config's full step count from its initial state, logging Nu / mass / max|uH| every so many steps")
+    ap.add_argument("--force-slabs", action="store_true",
+                    help="run the y-slab driver of N > 1 even with one rank (one slab, walls on both faces): a check of that code path")
     ap.add_argument("--pop-precision", type=int, default=64, choices=[64, 32],
                     help="storage of the populations in HBM (32: bandwidth study of BASELINE config 5; arithmetic stays fp64)")
     args = ap.parse_args()
