@@ -3,7 +3,7 @@
  *
  * The operation is the per-time-step update of TLBfind (arXiv 2109.12565); citations are
  * "PAPER L<line>" into /root/reference/PAPER.md plus the equation / section they fall in.
- * Readings R1..R30 of silent or garbled passages are listed in DESIGN.md.
+ * Readings R1..R31 of silent or garbled passages are listed in DESIGN.md.
  *
  * One step (tlb_step) computes, for every fluid site, from time-t populations only (R13):
  *   moments            rho_l = sum_i f_l,i ; T = sum_i g_i ; j = sum_l,i c_i f_l,i     Eqs. (4),(5),(17) L76-80, L165
@@ -171,6 +171,19 @@ int tlb_perturb_velocity(tlb_handle* h, double amplitude);
  * of the same nx, ny (the obstacle mask is not part of a dump: set it first).  Synchronise; TLB_EIO on a file error. */
 int tlb_write_checkpoint(tlb_handle* h, const char* dir, int32_t index);
 int tlb_read_checkpoint(tlb_handle* h, const char* dir, int32_t index);
+
+/* Field files of Tables C.9 / C.10 (L510-561) for the current state, written from the host after one read-back per field.
+ * `what` is a sum of TLB_OUT_* flags; <i> = index:
+ *   TLB_OUT_DENSITY      firstdensity.<i>.dat, seconddensity.<i>.dat      rho_A, rho_B
+ *   TLB_OUT_TEMPERATURE  temperature.<i>.dat                              T
+ *   TLB_OUT_VELOCITY     veloconf.<i>.dat, u_av.<i>.dat                   u^(H) (two columns), its x-average of u_x per row
+ *   TLB_OUT_STRESS       Ptot_xy.<i>.dat, Pxy_av.<i>.dat                  P_xy (R21), its x-average per row
+ * The paper names the files, not their format; reading R31: ASCII, one line "x y value" per site (velocity: "x y u_x
+ * u_y"; the averages: "y value"), x fastest, a blank line after every lattice row, numbers printed with 17 significant
+ * digits (they read back to the same doubles).  vtk != 0 adds <name>.<i>.vtk for the fields (legacy ASCII
+ * STRUCTURED_POINTS, "write vtk file" of Table C.9).  Synchronises; TLB_EIO on a file error; TLB_EINVAL on slab handles. */
+enum { TLB_OUT_DENSITY = 1, TLB_OUT_TEMPERATURE = 2, TLB_OUT_VELOCITY = 4, TLB_OUT_STRESS = 8 };
+int tlb_write_fields(tlb_handle* h, const char* dir, int32_t index, int32_t what, int32_t vtk);
 
 /* Arbitrary obstacle mask [ny][nx], non-zero = solid (flag field, L286).  Resets the state. */
 int tlb_set_solid(tlb_handle* h, const uint8_t* solid);

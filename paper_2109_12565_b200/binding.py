@@ -21,7 +21,7 @@ TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT, TLB_EIO = 0, -1, -2, 
 # every symbol include/tlb.h declares
 SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_slab_workspace_bytes",
            "tlb_create_slab", "tlb_slab_layout", "tlb_halo_bytes", "tlb_seg_rows", "tlb_init", "tlb_init_honeycomb",
-           "tlb_set_rough_walls", "tlb_perturb_velocity", "tlb_write_checkpoint", "tlb_read_checkpoint", "tlb_set_solid",
+           "tlb_set_rough_walls", "tlb_perturb_velocity", "tlb_write_checkpoint", "tlb_read_checkpoint", "tlb_write_fields", "tlb_set_solid",
            "tlb_set_solid_host", "tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations",
            "tlb_get_populations", "tlb_set_populations_host", "tlb_get_populations_host", "tlb_step",
            "tlb_slab_step_edges", "tlb_slab_step_interior", "tlb_slab_step_finish", "tlb_halo_pack", "tlb_halo_unpack",
@@ -98,6 +98,7 @@ def load_library():
     lib.tlb_perturb_velocity.argtypes = [vp, ctypes.c_double]
     lib.tlb_write_checkpoint.argtypes = [vp, ctypes.c_char_p, i32]
     lib.tlb_read_checkpoint.argtypes = [vp, ctypes.c_char_p, i32]
+    lib.tlb_write_fields.argtypes = [vp, ctypes.c_char_p, i32, i32, i32]
     lib.tlb_set_solid.argtypes = [vp, dp]
     lib.tlb_set_solid_host.argtypes = [vp, dp]
     for name in ("tlb_set_fields", "tlb_set_fields_host", "tlb_set_populations", "tlb_get_populations",
@@ -292,6 +293,12 @@ class TLB:
 
     def write_checkpoint(self, directory, index=0):
         self._chk(self.lib.tlb_write_checkpoint(self.h, os.fsencode(directory), int(index)))
+
+    OUT_DENSITY, OUT_TEMPERATURE, OUT_VELOCITY, OUT_STRESS = 1, 2, 4, 8
+
+    def write_fields(self, directory, index=0, what=15, vtk=False):
+        """The field files of Tables C.9 / C.10 (firstdensity.<i>.dat, ..., Pxy_av.<i>.dat; reading R31)."""
+        self._chk(self.lib.tlb_write_fields(self.h, os.fsencode(directory), int(index), int(what), int(bool(vtk))))
 
     def read_checkpoint(self, directory, index=0):
         self._chk(self.lib.tlb_read_checkpoint(self.h, os.fsencode(directory), int(index)))

@@ -666,6 +666,78 @@ int tlb_read_checkpoint(tlb_handle* h, const char* dir, int32_t index) {
   return tlb_set_populations_host(h, buf.data(), buf.data() + n9, buf.data() + 2 * n9);
 }
 
+// ---- field files (Tables C.9, C.10; reading R31): plain host I/O after a read-back ----
+static bool write_dat(const std::string& path, int nx, int ny, const double* a, const double* b) {
+  FILE* f = std::fopen(path.c_str(), "w");
+  if (!f) return false;
+  bool ok = true;
+  for (int y = 0; y < ny && ok; y++) {
+    for (int x = 0; x < nx; x++) {
+      const size_t q = (size_t)y * nx + x;
+      const int r = b ? std::fprintf(f, "%d %d %.17g %.17g\n", x, y, a[q], b[q]) : std::fprintf(f, "%d %d %.17g\n", x, y, a[q]);
+      if (r < 0) { ok = false; break; }
+    }
+    if (ok && std::fputc('\n', f) == EOF) ok = false;
+  }
+  return std::fclose(f) == 0 && ok;
+}
+static bool write_profile(const std::string& path, int ny, const double* a) {
+  FILE* f = std::fopen(path.c_str(), "w");
+  if (!f) return false;
+  bool ok = true;
+  for (int y = 0; y < ny && ok; y++) ok = std::fprintf(f, "%d %.17g\n", y, a[y]) >= 0;
+  return std::fclose(f) == 0 && ok;
+}
+static bool write_vtk(const std::string& path, const char* name, int nx, int ny, const double* a, const double* b) {
+  FILE* f = std::fopen(path.c_str(), "w");
+  if (!f) return false;
+  bool ok = std::fprintf(f, "# vtk DataFile Version 3.0\n%s\nASCII\nDATASET STRUCTURED_POINTS\nDIMENSIONS %d %d 1\n"
+                            "ORIGIN 0 0 0\nSPACING 1 1 1\nPOINT_DATA %lld\n", name, nx, ny, (long long)nx * ny) >= 0;
+  if (ok) ok = (b ? std::fprintf(f, "VECTORS %s double\n", name) : std::fprintf(f, "SCALARS %s double 1\nLOOKUP_TABLE default\n", name)) >= 0;
+  for (size_t q = 0; q < (size_t)nx * ny && ok; q++)
+    ok = (b ? std::fprintf(f, "%.17g %.17g 0\n", a[q], b[q]) : std::fprintf(f, "%.17g\n", a[q])) >= 0;
+  return std::fclose(f) == 0 && ok;
+}
+
+int tlb_write_fields(tlb_handle* h, const char* dir, int32_t index, int32_t what, int32_t vtk) {
+  if (!h || !dir || what < 0 || what > 15) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
+  const int nx = h->d.nx, ny = h->d.ny;
+  const size_t n = (size_t)nx * ny;
+  std::vector<double> a, b;
+  try { a.resize(2 * n); b.resize((size_t)ny > n ? (size_t)ny : n); } catch (...) { return TLB_EINVAL; }
+  const std::string base = std::string(dir) + "/", tag = "." + std::to_string(index);
+  auto field = [&](const char* name, const double* p, const double* q) {
+    if (!write_dat(base + name + tag + ".dat", nx, ny, p, q)) return false;
+    return !vtk || write_vtk(base + name + tag + ".vtk", name, nx, ny, p, q);
+  };
+  int rc;
+  if (what & (TLB_OUT_DENSITY | TLB_OUT_TEMPERATURE | TLB_OUT_VELOCITY)) {
+    if (what & TLB_OUT_DENSITY) {
+      if ((rc = tlb_fields_host(h, a.data(), b.data(), nullptr, nullptr)) != TLB_OK) return rc;
+      if (!field("firstdensity", a.data(), nullptr) || !field("seconddensity", b.data(), nullptr)) return TLB_EIO;
+    }
+    if (what & TLB_OUT_TEMPERATURE) {
+      if ((rc = tlb_fields_host(h, nullptr, nullptr, nullptr, a.data())) != TLB_OK) return rc;
+      if (!field("temperature", a.data(), nullptr)) return TLB_EIO;
+    }
+    if (what & TLB_OUT_VELOCITY) {
+      if ((rc = tlb_fields_host(h, nullptr, nullptr, a.data(), nullptr)) != TLB_OK) return rc;
+      if (!field("veloconf", a.data(), a.data() + n)) return TLB_EIO;
+      if ((rc = tlb_x_average_host(h, b.data())) != TLB_OK) return rc;
+      if (!write_profile(base + "u_av" + tag + ".dat", ny, b.data())) return TLB_EIO;
+    }
+  }
+  if (what & TLB_OUT_STRESS) {
+    if ((rc = tlb_stress_xy_host(h, a.data())) != TLB_OK) return rc;
+    if (!field("Ptot_xy", a.data(), nullptr)) return TLB_EIO;
+    if ((rc = tlb_x_average_stress_host(h, b.data())) != TLB_OK) return rc;
+    if (!write_profile(base + "Pxy_av" + tag + ".dat", ny, b.data())) return TLB_EIO;
+  }
+  return TLB_OK;
+}
+
 int tlb_step(tlb_handle* h, int64_t n) {
   if (!h || n < 0) return TLB_EINVAL;
   if (h->halo_lo || h->halo_hi) return TLB_EINVAL;  // a slab with halo rows steps through the tlb_slab_step_* calls

@@ -160,3 +160,40 @@ def test_checkpoint_restart(tlbmod, oracle_mod, tmp_path, prec):
     with pytest.raises(tlbmod.TLBError) as e:
         t3.read_checkpoint(d, 3)
     assert e.value.code == tlbmod.TLB_EIO
+
+
+def test_write_fields_round_trip(tlbmod, tmp_path):
+    """Tables C.9 / C.10 (reading R31): the ASCII files read back to exactly the arrays of tlb_fields, tlb_x_average,
+    tlb_stress_xy and tlb_x_average_stress (17 significant digits), in the documented order; the .vtk headers are
+    legacy STRUCTURED_POINTS."""
+    cfg = dict(inputs.config(1, "paper"), nx=96, ny=40, posts=(4, 4, 16))
+    cfg["init"] = dict(cfg["init"], n_droplets=5)
+    nx, ny = cfg["nx"], cfg["ny"]
+    t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
+    t.init(3)
+    t.step(25)
+    d = str(tmp_path)
+    t.write_fields(d, 7, what=15, vtk=True)
+    rA, rB, u, T = [_np(a) for a in t.fields()]
+    expect = {"firstdensity": [rA], "seconddensity": [rB], "temperature": [T], "veloconf": [u[0], u[1]], "Ptot_xy": [_np(t.stress_xy())]}
+    X, Y = np.meshgrid(np.arange(nx), np.arange(ny))
+    for name, arrs in expect.items():
+        m = np.loadtxt(os.path.join(d, "%s.7.dat" % name))
+        assert m.shape == (nx * ny, 2 + len(arrs))
+        assert (m[:, 0] == X.ravel()).all() and (m[:, 1] == Y.ravel()).all()
+        for k, a in enumerate(arrs):
+            assert (m[:, 2 + k] == a.ravel()).all(), name
+        raw = open(os.path.join(d, "%s.7.dat" % name)).read().split("\n")
+        assert raw[nx] == "" and raw[nx + 1].startswith("0 1 ")          # a blank line after every lattice row
+        head = open(os.path.join(d, "%s.7.vtk" % name)).read().split("\n")[:10]
+        assert head[0].startswith("# vtk DataFile") and head[3] == "DATASET STRUCTURED_POINTS" and head[4] == "DIMENSIONS %d %d 1" % (nx, ny)
+        assert head[8] == ("VECTORS %s double" % name if len(arrs) == 2 else "SCALARS %s double 1" % name)
+    for name, a in (("u_av", _np(t.x_average())), ("Pxy_av", _np(t.x_average_stress()))):
+        m = np.loadtxt(os.path.join(d, "%s.7.dat" % name))
+        assert m.shape == (ny, 2) and (m[:, 0] == np.arange(ny)).all() and (m[:, 1] == a).all()
+    # only what was asked for is written
+    t.write_fields(d, 8, what=t.OUT_TEMPERATURE)
+    assert sorted(f for f in os.listdir(d) if ".8." in f) == ["temperature.8.dat"]
+    with pytest.raises(tlbmod.TLBError) as e:
+        t.write_fields(os.path.join(d, "missing"), 9)
+    assert e.value.code == tlbmod.TLB_EIO
