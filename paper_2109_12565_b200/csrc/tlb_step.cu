@@ -89,14 +89,16 @@ __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* map, int c0, 
 __device__ __forceinline__ void prefetch_l2(const void* src, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(__cvta_generic_to_global(src)), "r"(bytes) : "memory");
 }
+// (L1 may keep the line: the x-shifted loads of neighbouring lanes and warps touch every line twice; measured -1.6 %
+// sustained against L1::no_allocate)
 __device__ __forceinline__ double ldg_stream(const double* a, uint64_t policy) {
   double v;
-  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(policy));
+  asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(v) : "l"(a), "l"(policy));
   return v;
 }
 __device__ __forceinline__ double ldg_stream(const float* a, uint64_t policy) {
   float v;
-  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(a), "l"(policy));
+  asm volatile("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(v) : "l"(a), "l"(policy));
   return (double)v;
 }
 __device__ __forceinline__ void stg_stream(double* a, double v, uint64_t policy) {
