@@ -3,7 +3,7 @@
  *
  * The operation is the per-time-step update of TLBfind (arXiv 2109.12565); citations are
  * "PAPER L<line>" into /root/reference/PAPER.md plus the equation / section they fall in.
- * Readings R1..R31 of silent or garbled passages are listed in DESIGN.md.
+ * Readings R1..R32 of silent or garbled passages are listed in DESIGN.md.
  *
  * One step (tlb_step) computes, for every fluid site, from time-t populations only (R13):
  *   moments            rho_l = sum_i f_l,i ; T = sum_i g_i ; j = sum_l,i c_i f_l,i     Eqs. (4),(5),(17) L76-80, L165

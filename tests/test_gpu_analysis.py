@@ -218,3 +218,55 @@ def test_droplet_nusselt_parity(tlbmod, oracle_mod):
     onu = o.droplet_nusselt(ostats[:, 2:4])
     assert np.abs(nu - onu).max() <= 1e-12 * max(1.0, np.abs(onu).max())
     assert np.abs(onu).max() > 0.1
+
+
+def test_delaunay_monitor_files(tlbmod, oracle_mod, tmp_path):
+    """The run-time monitor of Table C.12 (monitor.py, reading R32): a honeycomb emulsion checked every 40 steps (time
+    sequences, frame files that read back to what the analysis calls return and to the oracle's analysis of the same
+    state), then two hand-made frames of a sheared arrangement whose diagonals flip (events in the trigger directory)."""
+    import torch
+    from paper_2109_12565_b200 import monitor
+    cfg = dict(inputs.config(1, "paper"), nx=192, ny=96)
+    cfg["init"] = dict(cfg["init"], droplet_radius=8.0)
+    nx, ny = cfg["nx"], cfg["ny"]
+    t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
+    t.init_honeycomb(6, 3, 5)
+    B_th = 0.5 * (cfg["init"]["rho_in"] + cfg["init"]["rho_out"])
+    mon = monitor.DelaunayMonitor(t, B_th, str(tmp_path), max_droplets=64)
+    for k in range(3):
+        t.step(40)
+        ev = mon.check(40 * (k + 1))
+        assert len(ev) == 0          # a relaxing honeycomb does not rearrange
+    nb = np.loadtxt(tmp_path / "nBubblesOut")
+    nl = np.loadtxt(tmp_path / "nLinksOut")
+    assert (nb[:, 0] == [40, 80, 120]).all() and (nb[:, 1] == 18).all() and (nl[:, 1] == nl[0, 1]).all() and nl[0, 1] > 30
+    cen, links = monitor.read_frame(tmp_path / "delaunayNoTriggerDir" / "delaunayNowTime120")
+    fr = mon.frame(120)
+    assert (cen == _np(fr.centres)).all() and (links == _np(fr.links)).all()
+    # the oracle on the same state (through the populations) finds the same droplets, colouring and links
+    o = oracle_mod.Oracle(nx, ny, **cfg["params"])
+    o.set_solid(np.zeros((ny, nx), np.uint8))
+    o.set_populations(*[_np(p) for p in t.get_populations()])
+    _, ok, ostats = o.droplets(B_th, 64)
+    assert ok == 18 and (ostats[:, 2:4] == cen).all()
+    olinks, _ = oracle_mod.delaunay(oracle_mod.voronoi(nx, ny, 0, ostats[:, 2:4]), 0)
+    assert (olinks == links).all()
+    # two hand-made frames: every interior diagonal of a sheared square arrangement flips
+    NX, NY, cols, rows = 240, 192, 10, 8
+    t2 = tlbmod.TLB(NX, NY, periodic_y=1)
+    mon2 = monitor.DelaunayMonitor(t2, 0.0, str(tmp_path / "flip"))
+    frames = []
+    for step, shear in ((10, +0.06), (20, -0.06)):
+        c = _dev(t2, _sheared_grid(NX, NY, cols, rows, shear, 1), torch.float64)
+        colour = t2.voronoi(c)
+        lk, _ = t2.delaunay(colour, len(c))
+        frames.append(monitor.Frame(step, len(c), c, colour, lk))
+    assert len(mon2.record(frames[0])) == 0
+    ev = mon2.record(frames[1])
+    oev, one = oracle_mod.t1_events(_np(frames[0].links), _np(frames[1].links), np.arange(cols * rows, dtype=np.int32))
+    assert one == len(ev) == 80 and (ev == oev).all()
+    brk = np.loadtxt(tmp_path / "flip" / "delaunayTriggerDir" / "breakingLinks", dtype=int)
+    ari = np.loadtxt(tmp_path / "flip" / "delaunayTriggerDir" / "arisingLinks", dtype=int)
+    assert (brk[:, 0] == 20).all() and (brk[:, 1:] == ev[:, :2]).all() and (ari[:, 1:] == ev[:, 2:]).all()
+    pc, pl = monitor.read_frame(tmp_path / "flip" / "delaunayTriggerDir" / "delaunayPastTime20")
+    assert (pl == _np(frames[0].links)).all() and (pc == _np(frames[0].centres)).all()
