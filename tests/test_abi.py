@@ -88,3 +88,12 @@ def test_no_cpu_fallback(binding):
     h = ctypes.c_void_p()
     rc = lib.tlb_create(16, 16, ctypes.byref(p), 1 << 20, 1 << 30, None, ctypes.byref(h))
     assert rc == binding.TLB_ECUDA and not h.value
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/tlb.h is a C ABI: it compiles as C99 (no C++ or CUDA types in the signatures)."""
+    import subprocess
+    src = tmp_path / "t.c"
+    src.write_text('#include "tlb.h"\nint main(void) { tlb_params p; tlb_rough_walls r; (void)p; (void)r; return TLB_OK; }\n')
+    inc = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-pedantic", "-I", inc, "-c", str(src), "-o", str(tmp_path / "t.o")])
