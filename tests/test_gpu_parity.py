@@ -285,6 +285,42 @@ def test_full_size_windows_config4(tlbmod, oracle_mod, tau):
             assert np.abs(a[:, y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
 
 
+def test_large_ragged_lattice_windows(tlbmod, oracle_mod):
+    """A large lattice whose width is not a multiple of the strip width (3000 = 23 x 128 + 56) and whose height is odd:
+    the last strip is mostly padding, the periodic seam falls inside a strip's copy, the segments are cut at a row the
+    library chooses.  3 steps against oracle windows on the seam, the ragged strip edge x segment edge, and both walls."""
+    import torch
+    nx, ny, steps, m = 3000, 1501, 3, 12
+    cfg = dict(inputs.config(4), nx=nx, ny=ny)
+    cfg["init"] = dict(cfg["init"], n_droplets=1500)
+    solid, rA, rB, T = inputs.make_config_inputs(cfg)
+    t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
+    t.init(cfg["seed"])
+    t.step(steps)
+    pops = t.get_populations()
+    seg = t.seg_rows()
+    assert 30 < seg < ny - 30
+    xe = 23 * 128  # first column of the ragged last strip
+    windows = [("seam", np.r_[np.arange(nx - 90, nx), np.arange(0, 70)], np.arange(700, 760), "bulk"),
+               ("ragged_edge", np.arange(xe - 70, xe + 56), np.arange(seg - 30, seg + 30), "bulk"),
+               ("bottom", np.arange(xe - 100, xe + 50), np.arange(0, 48), "wall_bottom"),
+               ("top", np.arange(2900, 3000), np.arange(ny - 48, ny), "wall_top")]
+    for name, xs, ys, kind in windows:
+        sub = np.ix_(ys, xs)
+        par = dict(cfg["params"], periodic_y=1 if kind == "bulk" else 0)
+        o = oracle_mod.Oracle(len(xs), len(ys), **par)
+        o.set_solid(np.ascontiguousarray(solid[sub]))
+        o.set_fields(np.ascontiguousarray(rA[sub]), np.ascontiguousarray(rB[sub]), np.ascontiguousarray(T[sub]))
+        o.step(steps)
+        y_lo = 0 if kind == "wall_bottom" else m
+        y_hi = len(ys) if kind == "wall_top" else len(ys) - m
+        idx_y = torch.as_tensor(ys[y_lo:y_hi], device=pops[0].device)
+        idx_x = torch.as_tensor(xs[m:len(xs) - m], device=pops[0].device)
+        for a, b in zip(o.get_populations(), pops):
+            g = b.index_select(1, idx_y).index_select(2, idx_x).cpu().numpy()
+            assert np.abs(a[:, y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
+
+
 def test_table_b8b_on_the_gpu(tlbmod):
     """The paper's own printed numbers through the CUDA path: rows of Table B.8(b) (PAPER.md L497-508,
     tests/golden/table_b8b.txt), 128x2 doubly periodic, Table B.8 parameters, two-layer start (R15),
