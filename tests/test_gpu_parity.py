@@ -321,6 +321,50 @@ def test_large_ragged_lattice_windows(tlbmod, oracle_mod):
             assert np.abs(a[:, y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
 
 
+def test_largest_lattice_windows(tlbmod, oracle_mod):
+    """16384 x 8192 = 134 M sites (64 GB of workspace, four times config 5): the 64-bit offsets, the tensor-map strides
+    and the grid of 128 strips x 74 segments at the far corner of the buffers.  6 steps; rho_A against oracle windows
+    next to the last row / last column, at the periodic seam on both walls, far from the origin."""
+    import torch
+    nx, ny, tile, steps = 16384, 8192, 512, 6
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 80e9:
+        pytest.skip("needs 80 GB of free device memory")
+    cfg = dict(inputs.config(5), nx=nx, ny=ny)
+    cfg["init"] = dict(cfg["init"], n_droplets=0)
+    t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
+    dev = t.device
+    rA, rB, _ = inputs.smooth_random_fields(tile, tile, 3, 1.0, 0.0)     # one seeded tile, repeated over the lattice
+    Trow = 1.0 - (np.arange(ny) + 0.5) / ny
+    reps = (ny // tile, nx // tile)
+    t.set_fields(torch.as_tensor(rA, device=dev).repeat(*reps), torch.as_tensor(rB, device=dev).repeat(*reps),
+                 torch.as_tensor(Trow, device=dev)[:, None].repeat(1, nx).contiguous())
+    t.step(steps)
+    got = t.fields()[0]
+    m = 3 * steps + 2
+    for name, xs, ys, kind in [("far_bulk", np.arange(16000, 16160), np.arange(7900, 7980), "bulk"),
+                               ("top_seam", np.arange(nx - 80, nx + 80) % nx, np.arange(ny - 60, ny), "wall_top"),
+                               ("bottom_seam", np.arange(-80, 80) % nx, np.arange(0, 60), "wall_bottom")]:
+        par = dict(cfg["params"], periodic_y=1 if kind == "bulk" else 0)
+        o = oracle_mod.Oracle(len(xs), len(ys), **par)
+        o.set_solid(np.zeros((len(ys), len(xs)), np.uint8))
+        o.set_fields(np.ascontiguousarray(rA[np.ix_(ys % tile, xs % tile)]), np.ascontiguousarray(rB[np.ix_(ys % tile, xs % tile)]),
+                     np.ascontiguousarray(np.repeat(Trow[ys][:, None], len(xs), 1)))
+        o.step(steps)
+        y_lo = 0 if kind == "wall_bottom" else m
+        y_hi = len(ys) if kind == "wall_top" else len(ys) - m
+        iy = torch.as_tensor(ys[y_lo:y_hi], device=dev)
+        ix = torch.as_tensor(xs[m:len(xs) - m], device=dev)
+        g = got.index_select(0, iy).index_select(1, ix).cpu().numpy()
+        assert np.abs(o.fields()[0][y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
+    ob = t.observables()
+    assert all(np.isfinite(v) for v in ob.values())
+    t.close()
+
+
 def test_table_b8b_on_the_gpu(tlbmod):
     """The paper's own printed numbers through the CUDA path: rows of Table B.8(b) (PAPER.md L497-508,
     tests/golden/table_b8b.txt), 128x2 doubly periodic, Table B.8 parameters, two-layer start (R15),
