@@ -285,6 +285,26 @@ def test_full_size_windows_config4(tlbmod, oracle_mod, tau):
             assert np.abs(a[:, y_lo:y_hi, m:len(xs) - m] - g).max() <= TOL, name
 
 
+@pytest.mark.parametrize("nx,ny,per", [(1, 1, 0), (1, 1, 1), (2, 1, 0), (1, 3, 1), (3, 2, 0), (5, 1, 1), (129, 2, 0)])
+def test_degenerate_lattices(tlbmod, oracle_mod, nx, ny, per):
+    """Lattices down to a single site (every neighbour is a periodic image or a wall node; one strip of padding, one
+    segment shorter than the pipeline): 20 steps and the observables against the oracle."""
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4, periodic_y=per)
+    k = np.arange(nx * ny)
+    rA = (0.5 + inputs.uniform(nx, 11, k)).reshape(ny, nx)
+    rB = (0.3 + inputs.uniform(ny, 12, k)).reshape(ny, nx)
+    T = inputs.uniform(7, 13, k).reshape(ny, nx)
+    o, t = _pair(tlbmod, oracle_mod, nx, ny, par, np.zeros((ny, nx), np.uint8))
+    o.set_fields(rA, rB, T)
+    t.set_fields(rA, rB, T)
+    o.step(20)
+    t.step(20)
+    assert _maxdiff(o, t) <= TOL
+    oo, ot = o.observables(), t.observables()
+    for key in oo:
+        assert abs(ot[key] - oo[key]) <= 1e-12 * max(1.0, abs(oo[key])), key
+
+
 def test_large_ragged_lattice_windows(tlbmod, oracle_mod):
     """A large lattice whose width is not a multiple of the strip width (3000 = 23 x 128 + 56) and whose height is odd:
     the last strip is mostly padding, the periodic seam falls inside a strip's copy, the segments are cut at a row the
