@@ -187,6 +187,14 @@ struct Smem {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// the same, returning how many arrivals the phase was still waiting for BEFORE this one (1: this was the last)
+__device__ __forceinline__ uint32_t mbar_arrive_pending(uint64_t* bar) {
+  uint64_t state;
+  uint32_t pending;
+  asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 %0, [%1];" : "=l"(state) : "r"(smem_u32(bar)) : "memory");
+  asm volatile("mbarrier.pending_count.b64 %0, %1;" : "=r"(pending) : "l"(state));
+  return pending;
+}
 __device__ __forceinline__ double pair(double v) { return __shfl_xor_sync(0xffffffffu, v, 1); }  // the other species' lane
 
 // BGK relaxation of one population towards the second-order equilibrium, Eqs. (2), (3) (c_s^2 = 1/3);
@@ -330,6 +338,26 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     gd = ldg_stream(reinterpret_cast<const ST*>(gp + 2 * planeB + rofs - co), pol);
   };
 
+  // L2 prefetch of the 9 thermal plane rows that phase 2 of row yp will load (one elected lane)
+  auto prefetch_g = [&](int yp) {
+    if (!(MODE == 1 || MODE == 3 || d.thermal) || yp >= y1) return;
+    int ym = yp - 1, yq = yp + 1;
+    if (PERIODIC) {
+      if (ym < 0) ym = ny - 1;
+      if (yq >= ny) yq = 0;
+    }
+    if (kTensor && (!PERIODIC || (yp > 0 && yp < ny - 1))) {
+      tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp, 0, 0);
+    } else {
+      const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
+#pragma unroll
+      for (int i = 0; i < 9; i++) {
+        const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
+        prefetch_l2(Sin + (18 + pslot(i)) * plane + o, kCopyW * kB);
+      }
+    }
+  };
+
   constexpr int kLag = TAU1 ? 3 : 2;  // rows between phase 1 and phase 2
   uint32_t parity = 0;  // one bit per slot
   for (int q = 0; q < q_end + (kLag - 2); q++) {
@@ -345,40 +373,17 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     const int y = r - kLag;     // row of phase 2
     const bool do2 = y >= y0;
     if (do2 && (MODE == 1 || MODE == 3 || d.thermal)) load_g(y);  // consumed after the force stencil (a row earlier measured slower)
-    // Re-arm the slot every warp left during the previous iteration (row q - 3) with row q + 1, one iteration ahead of its
-    // use; the warps take turns, and by now the others have long passed their arrive, so the wait does not spin.
-    // (TAU1: a slot is left when the iteration of its row ends; row q + 1 goes into the slot of row q - 2, free for a whole
-    // iteration.  Two rows ahead measured 8 % slower: the issuer then waits for the slowest warp of the previous row.)
-    constexpr int kLead1 = 1;
-    if (q >= (TAU1 ? 0 : 3) && wid == ((q - 1) & (kWarps - 1)) && lane == 0) {
-      if (TAU1) {
-        const int qi = q + kLead1;
-        if (qi < q_end) {
-          if (qi >= 3) mbar_wait(&sm.empty[slot_of(qi)], ((qi - 3) / 3) & 1u);
-          issue(qi);
-        }
-      } else {
-        mbar_wait(&sm.empty[(q + 1) & 3], ((q - 3) >> 2) & 1u);
-        if (q + 1 < q_end) issue(q + 1);
+    // tau = 1: a landed row is dead when the iteration of its row ends (every warp arrives on the slot's "empty" barrier
+    // there, after it has consumed what it loaded); the warps take turns re-arming: row q + 1 goes into the slot of row
+    // q - 2, free for a whole iteration, so the wait below does not spin.  (Two rows ahead measured 8 % slower: the
+    // issuer then waits for the slowest warp of the previous row.)
+    if (TAU1 && wid == ((q - 1) & (kWarps - 1)) && lane == 0) {
+      const int qi = q + 1;
+      if (qi < q_end) {
+        if (qi >= 3) mbar_wait(&sm.empty[slot_of(qi)], ((qi - 3) / 3) & 1u);
+        issue(qi);
       }
-      const int yp = y0 + q - 2 - kLag + kGPrefetchRows;  // phase 2 of row yp runs kGPrefetchRows iterations from now
-      if ((MODE == 1 || MODE == 3 || d.thermal) && yp < y1) {
-        int ym = yp - 1, yq = yp + 1;
-        if (PERIODIC) {
-          if (ym < 0) ym = ny - 1;
-          if (yq >= ny) yq = 0;
-        }
-        if (kTensor && (!PERIODIC || (yp > 0 && yp < ny - 1))) {
-          tma_prefetch_4d(&tm.g, kXL + x0 - kHX, yp, 0, 0);
-        } else {
-          const long long o0 = d.at(x0 - kHX, yp), om = d.at(x0 - kHX, ym), op = d.at(x0 - kHX, yq);
-#pragma unroll
-          for (int i = 0; i < 9; i++) {
-            const long long o = cy(i) == 0 ? o0 : (cy(i) > 0 ? om : op);
-            prefetch_l2(Sin + (18 + pslot(i)) * plane + o, kCopyW * kB);
-          }
-        }
-      }
+      prefetch_g(y0 + q - 2 - kLag + kGPrefetchRows);  // phase 2 of that row runs kGPrefetchRows iterations from now
     }
     // ---- (1) rho_s, psi^s_s of row r (Eqs. (4), (12)); wall values at solid / out-of-domain nodes (L155, R9)
     if (valid) {
@@ -439,10 +444,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 #pragma unroll
       for (int i = 0; i < 9; i++) f[i] = (double)fs[pslot(i) * kSW - cx(i)];
     }
-    if (!TAU1) {
-      __syncwarp();  // ring row r of this warp is complete; this warp has read slot2 for the last time
-      if (lane == 0 && q >= 2) mbar_arrive(&sm.empty[slot2]);
-    }
+    if (!TAU1) __syncwarp();  // ring row r of this warp is complete
     if (do2) {
 
     // ---- (2) collide row y = r - 2, whose stencil rows y-2..y+2 = r-4..r are resident
@@ -637,6 +639,16 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     if (TAU1) {
       __syncwarp();  // ring row r of this warp is complete; this warp has read the slot of row r for the last time
       if (lane == 0 && p1) mbar_arrive(&sm.empty[slot]);
+    } else if (q >= 2) {
+      // General tau: the populations of row r - 2 were read from slot2 for the collision above.  The arrive sits HERE, after
+      // the values have been consumed: placed right behind the loads (they may still be queued in the LSU) it let the
+      // re-arming copy overwrite a slot that was still being read -- a rare, run-to-run race.  Whoever arrives last
+      // re-arms the slot with row q + 2 at once: nobody waits, and the copy has a whole iteration to land.
+      __syncwarp();
+      if (lane == 0 && mbar_arrive_pending(&sm.empty[slot2]) == 1) {
+        if (q + 2 < q_end) issue(q + 2);
+        prefetch_g(y0 + q - 3 + kGPrefetchRows);  // phase 2 of that row runs kGPrefetchRows iterations after the next one starts
+      }
     }
   }
   if (MODE == 3) {
