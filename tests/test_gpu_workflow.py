@@ -197,3 +197,33 @@ def test_write_fields_round_trip(tlbmod, tmp_path):
     with pytest.raises(tlbmod.TLBError) as e:
         t.write_fields(os.path.join(d, "missing"), 9)
     assert e.value.code == tlbmod.TLB_EIO
+
+
+def test_bench_json_contract(tlbmod):
+    """bench.py prints ONE JSON line with the keys the driver reads (small config, short run)."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--config", "1", "--steps", "20", "--warmup", "3"],
+                         capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "roofline", "cpu_baseline", "e2e", "gpu_launches", "clocks"):
+        assert key in d, key
+    assert d["metric"] == "MLUPS" and d["unit"] == "MLUPS" and d["n_gpus"] == 1 and d["steps"] == 20 and d["dtype"] == "f64"
+    assert d["higher_is_better"] is True and d["vs_baseline"] is None and d["data"] == "synthetic"
+    assert d["config"]["workload"].startswith("config1") and "model" not in d["config"]
+    assert d["gpu_launches"] == 40 and d["value"] > 0
+    r = d["roofline"]
+    for key in ("bound", "achieved", "peak", "unit", "frac", "traffic"):
+        assert key in r, key
+    assert r["bound"] == "hbm" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 0 and "sample" in c
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 3 * 8 * 128 * 64 and e["d2h_bytes_per_step"] == 32
+    assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
