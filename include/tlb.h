@@ -75,7 +75,8 @@ enum {
   TLB_ESTATE = -2,     /* step / fields / observables before any state was set                   */
   TLB_ECUDA = -3,      /* a CUDA call failed (sticky on the handle); see tlb_last_cuda_error      */
   TLB_EPLACEMENT = -4, /* tlb_init could not place n_droplets within 1000 * n_droplets candidates */
-  TLB_EIO = -5         /* a checkpoint file could not be opened, or has the wrong size              */
+  TLB_EIO = -5,        /* a checkpoint file could not be opened, or has the wrong size              */
+  TLB_ELIMIT = -6      /* a size beyond the fixed capacity of tlb_t1_events_static                 */
 };
 
 /* POD, passed by pointer, copied by tlb_create. */
@@ -317,6 +318,34 @@ int tlb_t1_events(tlb_handle* h, const int32_t* links_past, int32_t n_past, cons
                   const int32_t* map, int32_t n_map, int32_t n_droplets, int32_t max_events, int32_t* n_events,
                   int32_t* events);
 int tlb_droplet_nusselt(tlb_handle* h, const double* centres, int32_t n, double* nu);
+
+/* tlb_t1_events for callers that cannot allocate device memory.  Every other call of this library works inside the
+ * workspace given to tlb_create, and tlb_t1_events keeps its adjacency tables there.  This variant needs no handle and
+ * no workspace, and it makes no cudaMalloc / cudaFree or other allocating call, ever: its tables live in a fixed array
+ * inside the library's device image (about 4.3 MB that every GPU which loads libtlb.so holds until the process ends).
+ * It is meant for
+ *   - tools that only compare two Delaunay link lists (the paper's deltaAnalysis, L338-341) and own no lattice;
+ *   - a monitor called from inside a time loop whose lattice was sized to fill the GPU: an allocation there can fail,
+ *     and even a successful cudaMalloc holds up all streams of the device while it runs;
+ *   - code hosted by an application that manages all device memory itself and does not let guests allocate.
+ * Arguments, outputs and their order are those of tlb_t1_events (R25, section 2.4) minus the handle: DEVICE
+ * pointers owned by the caller, nothing retained; the work is enqueued on `stream` (a cudaStream_t as void*, NULL =
+ * default stream) of the calling thread's CURRENT device and the call returns without synchronising.  The events are
+ * bit-identical to tlb_t1_events'.
+ * Limits: n_droplets <= TLB_T1_STATIC_MAX_DROPLETS, else TLB_ELIMIT and nothing is enqueued; if more than
+ * TLB_T1_STATIC_MAX_EVENTS events are found, *n_events = -1 (as on a table overflow).  n_past, n_now, n_map and
+ * max_events are not limited.
+ * One array serves every call in the process on a given GPU.  Each call clears, on its stream, the part it relies on,
+ * so consecutive calls on one stream are independent; two calls that may run at the same time on one GPU (different
+ * streams, or different threads) overwrite each other's tables and give garbage: serialise them.
+ * The first call on each device also loads the device code and looks the array up (cudaGetSymbolAddress); make that
+ * call before any stream capture begins.
+ * TLB_EINVAL for negative counts or missing pointers, TLB_ECUDA for a CUDA error (also one left pending by others). */
+#define TLB_T1_STATIC_MAX_DROPLETS 16384
+#define TLB_T1_STATIC_MAX_EVENTS 16384
+int tlb_t1_events_static(const int32_t* links_past, int32_t n_past, const int32_t* links_now, int32_t n_now,
+                         const int32_t* map, int32_t n_map, int32_t n_droplets, int32_t max_events, int32_t* n_events,
+                         int32_t* events, void* stream);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t tlb_launch_count(const tlb_handle* h);

@@ -12,11 +12,12 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB_PATH = os.path.join(_HERE, "libtlb.so")
-SOURCES = ["tlb_step.cu", "tlb_aux.cu", "tlb_analysis.cu", "tlb_api.cu"]
+SOURCES = ["tlb_step.cu", "tlb_aux.cu", "tlb_analysis.cu", "tlb_api.cu", "tlb_noalloc.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-shared"]
 
-TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT, TLB_EIO = 0, -1, -2, -3, -4, -5
+TLB_OK, TLB_EINVAL, TLB_ESTATE, TLB_ECUDA, TLB_EPLACEMENT, TLB_EIO, TLB_ELIMIT = 0, -1, -2, -3, -4, -5, -6
+T1_STATIC_MAX_DROPLETS = T1_STATIC_MAX_EVENTS = 16384  # TLB_T1_STATIC_MAX_* of include/tlb.h
 
 # every symbol include/tlb.h declares
 SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destroy", "tlb_slab_workspace_bytes",
@@ -30,6 +31,7 @@ SYMBOLS = ["tlb_default_params", "tlb_workspace_bytes", "tlb_create", "tlb_destr
            "tlb_observable_sums", "tlb_observables_from_sums", "tlb_x_average", "tlb_x_average_host",
            "tlb_stress_xy", "tlb_stress_xy_host", "tlb_x_average_stress", "tlb_x_average_stress_host",
            "tlb_droplets", "tlb_droplets_host", "tlb_voronoi", "tlb_delaunay", "tlb_droplet_match", "tlb_droplet_displacements", "tlb_t1_events",
+           "tlb_t1_events_static",
            "tlb_droplet_nusselt", "tlb_launch_count", "tlb_error_string", "tlb_last_cuda_error"]
 
 
@@ -131,6 +133,7 @@ def load_library():
     lib.tlb_droplet_match.argtypes = [vp, dp, dp, i32, dp]
     lib.tlb_droplet_displacements.argtypes = [vp, dp, dp, dp, i32, dp]
     lib.tlb_t1_events.argtypes = [vp, dp, i32, dp, i32, dp, i32, i32, i32, dp, dp]
+    lib.tlb_t1_events_static.argtypes = [dp, i32, dp, i32, dp, i32, i32, i32, dp, dp, vp]
     lib.tlb_droplet_nusselt.argtypes = [vp, dp, i32, dp]
     lib.tlb_launch_count.argtypes = [vp]
     lib.tlb_launch_count.restype = i64
@@ -156,6 +159,31 @@ def default_params(**overrides):
 
 def _ptr(t):
     return None if t is None else t.data_ptr()
+
+
+def t1_events_static(links_past, links_now, n_droplets, n_events, events, map_now_to_past=None, stream=None):
+    """tlb_t1_events_static: the T1 events between two Delaunay link lists without a TLB handle, a workspace or any
+    device allocation -- for tools that own no lattice, for monitors running beside a lattice that fills the GPU, and for
+    hosts that do not let guests allocate (include/tlb.h has the full story).  Nothing is allocated here either: the
+    caller passes the outputs, `n_events` (int32 [1]) and `events` (int32 [max_events][4]), next to the inputs
+    (contiguous int32 CUDA tensors on one device; `map_now_to_past` may be None).  The work goes on `stream` (default:
+    torch's current stream of that device) and is not synchronised.  At most T1_STATIC_MAX_DROPLETS droplets
+    (TLBError with code TLB_ELIMIT beyond).  All calls on one GPU share one scratch array: do not let two overlap."""
+    import torch
+    lib = load_library()
+    tensors = [t for t in (links_past, links_now, map_now_to_past, n_events, events) if t is not None]
+    for t in tensors:
+        if t.dtype != torch.int32 or not t.is_cuda or not t.is_contiguous() or t.device != n_events.device:
+            raise TLBError(TLB_EINVAL, "t1_events_static takes contiguous int32 CUDA tensors on one device")
+    if n_events.numel() < 1 or (events.numel() > 0 and (events.dim() != 2 or events.shape[1] != 4)):
+        raise TLBError(TLB_EINVAL, "n_events is int32 [1], events is int32 [max_events][4]")
+    with torch.cuda.device(n_events.device):  # the entry point works on the current device
+        st = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.tlb_t1_events_static(_ptr(links_past), int(links_past.shape[0]), _ptr(links_now), int(links_now.shape[0]),
+                                      _ptr(map_now_to_past), 0 if map_now_to_past is None else int(map_now_to_past.shape[0]),
+                                      int(n_droplets), int(events.shape[0]), n_events.data_ptr(), _ptr(events), st.cuda_stream)
+    if rc != TLB_OK:
+        raise TLBError(rc, lib.tlb_error_string(rc).decode())
 
 
 class TLB:

@@ -1114,6 +1114,7 @@ const char* tlb_error_string(int code) {
     case TLB_ECUDA: return "CUDA error (see tlb_last_cuda_error); there is no CPU fallback";
     case TLB_EPLACEMENT: return "tlb_init could not place n_droplets by random sequential addition";
     case TLB_EIO: return "checkpoint file missing, unreadable, unwritable or of another lattice size";
+    case TLB_ELIMIT: return "size beyond the fixed capacity of tlb_t1_events_static (TLB_T1_STATIC_MAX_DROPLETS droplets, 64 devices)";
   }
   return "unknown error code";
 }
