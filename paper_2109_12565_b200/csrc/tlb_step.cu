@@ -181,19 +181,20 @@ struct Smem {
   uint8_t flag[kWarps][kRingRows][kWR + 4];  // 1 = solid / wall node
   uint64_t full[kSlots];                     // mbarriers: row landed
   uint64_t empty[kSlots];                    // mbarriers: all kWarps warps have finished reading the slot
+  uint32_t ticket[kSlots];                   // general tau: arrivals per slot so far (elects the warp that re-arms it)
 };
 
 // release arrive of one thread on an mbarrier (the warp is done with the slot the barrier guards)
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-// the same, returning how many arrivals the phase was still waiting for BEFORE this one (1: this was the last)
-__device__ __forceinline__ uint32_t mbar_arrive_pending(uint64_t* bar) {
-  uint64_t state;
-  uint32_t pending;
-  asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 %0, [%1];" : "=l"(state) : "r"(smem_u32(bar)) : "memory");
-  asm volatile("mbarrier.pending_count.b64 %0, %1;" : "=r"(pending) : "l"(state));
-  return pending;
+// Election of the warp that re-arms a slot: a plain shared counter per slot, bumped by lane 0 of every warp AFTER its
+// arrive on the slot's "empty" barrier.  The warp that sees kWarps - 1 (mod kWarps) knows the other arrivals have been
+// made, so its acquiring wait on "empty" (below, before the copy is issued) falls through at once.
+__device__ __forceinline__ uint32_t slot_ticket(uint32_t* cnt) {
+  uint32_t old;
+  asm volatile("atom.relaxed.cta.shared::cta.add.u32 %0, [%1], 1;" : "=r"(old) : "r"(smem_u32(cnt)) : "memory");
+  return old;
 }
 __device__ __forceinline__ double pair(double v) { return __shfl_xor_sync(0xffffffffu, v, 1); }  // the other species' lane
 
@@ -248,7 +249,7 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
 
   if (t == 0) {
 #pragma unroll
-    for (int i = 0; i < kS; i++) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], kWarps); }
+    for (int i = 0; i < kS; i++) { mbar_init(&sm.full[i], 1); mbar_init(&sm.empty[i], kWarps); sm.ticket[i] = 0; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -492,6 +493,11 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
     } else {
       jxl = ((f[1] - f[3]) + (f[5] - f[6])) + (f[8] - f[7]);
       jyl = ((f[2] - f[4]) + (f[5] - f[7])) + (f[6] - f[8]);
+      // The slot these nine values came from is handed back at the end of the iteration (the arrive below).  Pin that order
+      // down instead of leaving it to where the compiler happens to put things: this statement needs all nine loads
+      // complete (j depends on f_1..f_8), and volatile asm statements keep their program order, so no load of slot2 can
+      // be scheduled behind the arrive -- also in the modes where the values only feed register accumulators.
+      asm volatile("" ::"d"(f[0]), "d"(jxl), "d"(jyl));
     }
     const double jx = jxl + pair(jxl), jy = jyl + pair(jyl);
     // Eq. (22) buoyancy (R12) and the x-acceleration extension
@@ -640,14 +646,19 @@ fused_kernel(const Dev d, const ST* __restrict__ Sin, ST* __restrict__ Sout, int
       __syncwarp();  // ring row r of this warp is complete; this warp has read the slot of row r for the last time
       if (lane == 0 && p1) mbar_arrive(&sm.empty[slot]);
     } else if (q >= 2) {
-      // General tau: the populations of row r - 2 were read from slot2 for the collision above.  The arrive sits HERE, after
-      // the values have been consumed: placed right behind the loads (they may still be queued in the LSU) it let the
-      // re-arming copy overwrite a slot that was still being read -- a rare, run-to-run race.  Whoever arrives last
-      // re-arms the slot with row q + 2 at once: nobody waits, and the copy has a whole iteration to land.
+      // General tau: the populations of row r - 2 were read from slot2 for the collision above; every warp hands the slot
+      // back HERE, after the values have been consumed (see the asm next to j above).  The warp whose ticket shows that it
+      // is the last of the kWarps re-arms the slot with row q + 2 at once: the copy has a whole iteration to land.  Before
+      // it issues the copy it waits on "empty" like the tau = 1 issuer does -- the wait cannot block (all arrivals are
+      // in), it is there for its acquire: the other warps' reads of the slot are ordered before the copy that overwrites it.
       __syncwarp();
-      if (lane == 0 && mbar_arrive_pending(&sm.empty[slot2]) == 1) {
-        if (q + 2 < q_end) issue(q + 2);
-        prefetch_g(y0 + q - 3 + kGPrefetchRows);  // phase 2 of that row runs kGPrefetchRows iterations after the next one starts
+      if (lane == 0) {
+        mbar_arrive(&sm.empty[slot2]);
+        if ((slot_ticket(&sm.ticket[slot2]) & (kWarps - 1)) == kWarps - 1) {
+          mbar_wait(&sm.empty[slot2], ((q - 2) >> 2) & 1u);  // completion number (q - 2) / 4 of this slot's barrier
+          if (q + 2 < q_end) issue(q + 2);
+          prefetch_g(y0 + q - 3 + kGPrefetchRows);  // phase 2 of that row runs kGPrefetchRows iterations after the next one starts
+        }
       }
     }
   }

@@ -305,27 +305,34 @@ def test_degenerate_lattices(tlbmod, oracle_mod, nx, ny, per):
         assert abs(ot[key] - oo[key]) <= 1e-12 * max(1.0, abs(oo[key])), key
 
 
-@pytest.mark.parametrize("tau", [1.0, 0.9])
-def test_repeated_runs_are_bit_identical(tlbmod, tau):
-    """Regression test of the slot hand-over: the step has no order-dependent arithmetic, so two runs from the same seed
-    must agree bit for bit -- at full size, in the launch configuration bench.py times, for both kernel instantiations
-    and for the non-stepping modes (fields, stress, observables).  A slot re-armed while a warp was still reading it
-    showed up here as differences of order 0.1 at a fraction of a per cent of the sites after 5 steps."""
-    import hashlib
+@pytest.mark.parametrize("tau,prec", [(1.0, 64), (0.9, 64), (1.0, 32), (0.9, 32)])
+def test_repeated_runs_are_bit_identical(tlbmod, tau, prec):
+    """Regression test of the slot hand-over: the step has no order-dependent arithmetic, so runs from the same seed
+    must agree bit for bit -- at full size, in the launch configuration bench.py times, for both kernel instantiations,
+    both storage precisions and the non-stepping modes (fields, stress, observables: the general-tau kernel in modes 1,
+    2, 3).  A slot re-armed while a warp was still reading it showed up here as differences of order 0.1 at a fraction
+    of a per cent of the sites after 5 steps.  24 runs per case; the digests are wrapping integer sums of the bit
+    patterns, taken on the device."""
+    import torch
     cfg = inputs.config(4)
-    cfg["params"] = dict(cfg["params"], tau=tau)
-    digests = []
-    for _ in range(3):
-        t = tlbmod.TLB(cfg["nx"], cfg["ny"], params=tlbmod.params_from_config(cfg))
+    cfg["params"] = dict(cfg["params"], tau=tau, pop_precision=prec)
+    t = tlbmod.TLB(cfg["nx"], cfg["ny"], params=tlbmod.params_from_config(cfg))
+
+    def digest(a):
+        v = a.contiguous().view(torch.int64).reshape(-1)
+        return (int(v.sum().item()), int(v[::3].sum().item()), int(v[1::7].sum().item()))
+
+    digests = set()
+    for run in range(24):
         t.init(cfg["seed"])
         t.step(40)
-        h = hashlib.sha256()
+        d = []
         for a in list(t.get_populations()) + list(t.fields()) + [t.stress_xy()]:
-            h.update(a.cpu().numpy().tobytes())
-        h.update(repr(sorted(t.observables().items())).encode())
-        digests.append(h.hexdigest())
-        t.close()
-    assert len(set(digests)) == 1, digests
+            d.append(digest(a))
+        d.append(repr(sorted(t.observables().items())))
+        digests.add(tuple(d))
+        assert len(digests) == 1, "run %d differs from the runs before it" % run
+    t.close()
 
 
 def test_large_ragged_lattice_windows(tlbmod, oracle_mod):
