@@ -181,8 +181,9 @@ int tlb_read_checkpoint(tlb_handle* h, const char* dir, int32_t index);
  *   TLB_OUT_STRESS       Ptot_xy.<i>.dat, Pxy_av.<i>.dat                  P_xy (R21), its x-average per row
  * The paper names the files, not their format; reading R31: ASCII, one line "x y value" per site (velocity: "x y u_x
  * u_y"; the averages: "y value"), x fastest, a blank line after every lattice row, numbers printed with 17 significant
- * digits (they read back to the same doubles).  vtk != 0 adds <name>.<i>.vtk for the fields (legacy ASCII
- * STRUCTURED_POINTS, "write vtk file" of Table C.9).  Synchronises; TLB_EIO on a file error; TLB_EINVAL on slab handles. */
+ * digits (they read back to the same doubles).  vtk != 0 adds <name>.<i>.vtk for the fields ("binary VTK 2.0", L244-246:
+ * legacy "# vtk DataFile Version 2.0" header, BINARY, STRUCTURED_POINTS, one SCALARS / VECTORS array of big-endian doubles;
+ * "write vtk file" of Table C.9).  Synchronises; TLB_EIO on a file error; TLB_EINVAL on slab handles. */
 enum { TLB_OUT_DENSITY = 1, TLB_OUT_TEMPERATURE = 2, TLB_OUT_VELOCITY = 4, TLB_OUT_STRESS = 8 };
 int tlb_write_fields(tlb_handle* h, const char* dir, int32_t index, int32_t what, int32_t vtk);
 
@@ -194,7 +195,8 @@ int tlb_set_solid_host(tlb_handle* h, const uint8_t* solid);
 int tlb_set_fields(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T);
 int tlb_set_fields_host(tlb_handle* h, const double* rho_A, const double* rho_B, const double* T);
 
-/* State from / to time-t populations, each [9][ny][nx] (checkpoint / restart, L252). */
+/* State from / to time-t populations, each [9][ny][nx] (checkpoint / restart, L252).  tlb_get_populations(_host)
+ * return TLB_ESTATE between tlb_slab_step_edges and tlb_slab_step_finish (the staging area is the buffer being written). */
 int tlb_set_populations(tlb_handle* h, const double* fA, const double* fB, const double* g);
 int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g);
 int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, const double* g);

@@ -575,7 +575,7 @@ int tlb_set_populations(tlb_handle* h, const double* fA, const double* fB, const
 
 int tlb_get_populations(tlb_handle* h, double* fA, double* fB, double* g) {
   if (!h) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
   TLB_ENTER(h);
   h->launches += launch_gather(h->d, h->S[h->cur], fA, fB, g, h->st);
   return check(h);
@@ -601,7 +601,9 @@ int tlb_set_populations_host(tlb_handle* h, const double* fA, const double* fB, 
 
 int tlb_get_populations_host(tlb_handle* h, double* fA, double* fB, double* g) {
   if (!h || !fA || !fB || !g) return TLB_EINVAL;
-  if (!h->has_state) return TLB_ESTATE;
+  // while a slab step is open the other buffer holds the rows just computed and the halo rows being received:
+  // staging through it would corrupt the step
+  if (!h->has_state || h->step_open) return TLB_ESTATE;
   TLB_ENTER(h);
   const size_t n9 = 9 * (size_t)h->d.nx * h->d.ny;
   double* stage = h->stage ? h->stage : static_cast<double*>(h->S[1 - h->cur]);
@@ -688,14 +690,27 @@ static bool write_profile(const std::string& path, int ny, const double* a) {
   for (int y = 0; y < ny && ok; y++) ok = std::fprintf(f, "%d %.17g\n", y, a[y]) >= 0;
   return std::fclose(f) == 0 && ok;
 }
+// "binary VTK 2.0" (L244-246): legacy header, then the values as big-endian doubles (the byte order the legacy format fixes)
 static bool write_vtk(const std::string& path, const char* name, int nx, int ny, const double* a, const double* b) {
-  FILE* f = std::fopen(path.c_str(), "w");
+  FILE* f = std::fopen(path.c_str(), "wb");
   if (!f) return false;
-  bool ok = std::fprintf(f, "# vtk DataFile Version 3.0\n%s\nASCII\nDATASET STRUCTURED_POINTS\nDIMENSIONS %d %d 1\n"
+  bool ok = std::fprintf(f, "# vtk DataFile Version 2.0\n%s\nBINARY\nDATASET STRUCTURED_POINTS\nDIMENSIONS %d %d 1\n"
                             "ORIGIN 0 0 0\nSPACING 1 1 1\nPOINT_DATA %lld\n", name, nx, ny, (long long)nx * ny) >= 0;
   if (ok) ok = (b ? std::fprintf(f, "VECTORS %s double\n", name) : std::fprintf(f, "SCALARS %s double 1\nLOOKUP_TABLE default\n", name)) >= 0;
-  for (size_t q = 0; q < (size_t)nx * ny && ok; q++)
-    ok = (b ? std::fprintf(f, "%.17g %.17g 0\n", a[q], b[q]) : std::fprintf(f, "%.17g\n", a[q])) >= 0;
+  const size_t n = (size_t)nx * ny, per = b ? 3 : 1;
+  std::vector<unsigned char> out;
+  try { out.resize(n * per * 8); } catch (...) { std::fclose(f); return false; }
+  auto put = [&](size_t slot, double v) {
+    uint64_t u;
+    std::memcpy(&u, &v, 8);
+    for (int k = 0; k < 8; k++) out[slot * 8 + k] = (unsigned char)(u >> (56 - 8 * k));
+  };
+  for (size_t q = 0; q < n; q++) {
+    put(q * per, a[q]);
+    if (b) { put(q * per + 1, b[q]); put(q * per + 2, 0.0); }
+  }
+  if (ok) ok = std::fwrite(out.data(), 1, out.size(), f) == out.size();
+  if (ok) ok = std::fputc('\n', f) != EOF;
   return std::fclose(f) == 0 && ok;
 }
 
@@ -1082,6 +1097,7 @@ int tlb_t1_events(tlb_handle* h, const int32_t* links_past, int32_t n_past, cons
                   int32_t* events) {
   if (!h || !n_events || n_past < 0 || n_now < 0 || n_droplets < 0 || max_events < 0 || n_map < 0) return TLB_EINVAL;
   if ((n_past > 0 && !links_past) || (n_now > 0 && !links_now) || (max_events > 0 && !events)) return TLB_EINVAL;
+  if (h->slab) return TLB_EINVAL;
   const size_t N = (size_t)h->d.nx * h->d.ny;
   if (2 * (size_t)n_droplets * kMaxDegree > 2 * N || N < 8) return TLB_EINVAL;
   TLB_ENTER(h);

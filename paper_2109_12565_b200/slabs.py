@@ -62,8 +62,10 @@ def face_rows(lay, face, halo=HALO):
 
 def exchange(dist, send, recv, lo, hi, rank):
     """Move the packed faces: send[0] (my low rows) -> rank `lo`, send[1] (my high rows) -> rank `hi`; recv[0] <- what
-    `lo` sent upwards, recv[1] <- what `hi` sent downwards.  Tags tell the two directions apart when lo == hi
-    (two slabs of a periodic lattice).  A face whose neighbour is this rank itself (one slab of a periodic lattice)
+    `lo` sent upwards, recv[1] <- what `hi` sent downwards.  When lo == hi (two slabs of a periodic lattice) both
+    directions go to the same peer.  gloo tells them apart by the tags; NCCL ignores tags and pairs the k-th send to a
+    peer with the k-th receive that peer posts for this rank, so the pairing then rests on the ORDER below -- send up,
+    send down, receive the upward face, receive the downward face -- being the same on both ranks.  Keep it.  A face whose neighbour is this rank itself (one slab of a periodic lattice)
     is a local copy.  Returns when the receives have completed on the current stream / thread."""
     UP, DOWN = 0, 1
     ops = []

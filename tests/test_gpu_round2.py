@@ -31,16 +31,18 @@ def _gather_owned(slabs, arrays_per_slab):
     return np.concatenate([_np(s.owned(a)) for s, a in zip(slabs, arrays_per_slab)], axis=-2)
 
 
+@pytest.mark.parametrize("tau,tau_g", [(1.0, 1.0), (0.9, 0.8)])
 @pytest.mark.parametrize("geom,world", [("posts", 2), ("posts", 3), ("random_mask", 2), ("periodic_y_mask", 2),
                                         ("periodic_y_mask", 1), ("moving_walls", 4)])
-def test_slabs_match_one_handle_bit_for_bit(tlbmod, oracle_mod, geom, world):
+def test_slabs_match_one_handle_bit_for_bit(tlbmod, oracle_mod, geom, world, tau, tau_g):
     """2-4 slabs on ONE GPU (two+ handles, halo rows copied device to device through tlb_halo_pack / _unpack) against a
     single handle on the whole lattice: bit for bit after 10 steps, and <= 1e-12 from the oracle.  Lattice spans two
-    strips with a ragged tail; posts / random obstacles cross the slab faces."""
+    strips with a ragged tail; posts / random obstacles cross the slab faces.  Both instantiations of the fused kernel
+    (tau = 1 with 3 slots; general tau with 4) run the 3-row edge launches and the split interior launch."""
     from paper_2109_12565_b200 import slabs as S
     nx, ny = 200, 46
     per = 1 if geom.startswith("periodic_y") else 0
-    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4, periodic_y=per)
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4, periodic_y=per, tau=tau, tau_g=tau_g)
     if geom == "moving_walls":
         par.update(u_wall_bottom=-0.02, u_wall_top=0.03)
     solid = np.zeros((ny, nx), np.uint8)
@@ -115,6 +117,14 @@ def test_slab_call_order_and_arguments(tlbmod):
     s.begin_step()
     assert lib.tlb_slab_step_edges(s.t.h) == tlbmod.TLB_ESTATE      # already open
     assert lib.tlb_fields(s.t.h, None, None, None, None) == tlbmod.TLB_ESTATE
+    # the population read-backs stage through the buffer the open step is writing: refused, state untouched
+    import torch
+    pops = [torch.zeros((9, s.t.ny, 64), dtype=torch.float64, device=s.t.device) for _ in range(3)]
+    assert lib.tlb_get_populations(s.t.h, *[p.data_ptr() for p in pops]) == tlbmod.TLB_ESTATE
+    host = [p.cpu().numpy() for p in pops]
+    assert lib.tlb_get_populations_host(s.t.h, *[h.ctypes.data for h in host]) == tlbmod.TLB_ESTATE
+    ne = torch.zeros(1, dtype=torch.int32, device=s.t.device)
+    assert lib.tlb_t1_events(s.t.h, None, 0, None, 0, None, 0, 0, 0, ne.data_ptr(), None) == tlbmod.TLB_EINVAL  # slab handle
     s.recv[1].copy_(s.send[1])
     s.end_step()
     with pytest.raises(tlbmod.TLBError):
@@ -341,12 +351,13 @@ def test_config2_long_run_observables(tlbmod, physics):
         print("config2[%s] step %6d  Nu %.9f  mass_A %.12e  mass_B %.12e  E %.6e  max|uH| %.4e" % ((physics,) + row))
 
 
-def test_slabs_staged_and_zero_copy_exchange_agree(tlbmod):
+@pytest.mark.parametrize("tau,tau_g", [(1.0, 1.0), (0.9, 0.8)])
+def test_slabs_staged_and_zero_copy_exchange_agree(tlbmod, tau, tau_g):
     """The two transports of the halo rows -- straight out of / into the population buffers (tlb_halo_region) and through
     tlb_halo_pack / _unpack buffers -- give bit-identical states; the regions are the documented rows."""
     from paper_2109_12565_b200 import slabs as S
     nx, ny, world = 200, 46, 3
-    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4)
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4, tau=tau, tau_g=tau_g)
     solid = inputs.post_mask(nx, ny, 4, 4, 16)
     solid[ny // 2 - 2:ny // 2 + 3, 30:37] = 1
     rA, rB, T = inputs.smooth_random_fields(nx, ny, 2, 0.5, -0.5)

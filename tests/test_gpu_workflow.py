@@ -164,8 +164,8 @@ def test_checkpoint_restart(tlbmod, oracle_mod, tmp_path, prec):
 
 def test_write_fields_round_trip(tlbmod, tmp_path):
     """Tables C.9 / C.10 (reading R31): the ASCII files read back to exactly the arrays of tlb_fields, tlb_x_average,
-    tlb_stress_xy and tlb_x_average_stress (17 significant digits), in the documented order; the .vtk headers are
-    legacy STRUCTURED_POINTS."""
+    tlb_stress_xy and tlb_x_average_stress (17 significant digits), in the documented order; the .vtk twins are
+    binary legacy VTK 2.0 STRUCTURED_POINTS whose big-endian doubles are those arrays."""
     cfg = dict(inputs.config(1, "paper"), nx=96, ny=40, posts=(4, 4, 16))
     cfg["init"] = dict(cfg["init"], n_droplets=5)
     nx, ny = cfg["nx"], cfg["ny"]
@@ -185,9 +185,17 @@ def test_write_fields_round_trip(tlbmod, tmp_path):
             assert (m[:, 2 + k] == a.ravel()).all(), name
         raw = open(os.path.join(d, "%s.7.dat" % name)).read().split("\n")
         assert raw[nx] == "" and raw[nx + 1].startswith("0 1 ")          # a blank line after every lattice row
-        head = open(os.path.join(d, "%s.7.vtk" % name)).read().split("\n")[:10]
-        assert head[0].startswith("# vtk DataFile") and head[3] == "DATASET STRUCTURED_POINTS" and head[4] == "DIMENSIONS %d %d 1" % (nx, ny)
-        assert head[8] == ("VECTORS %s double" % name if len(arrs) == 2 else "SCALARS %s double 1" % name)
+        blob = open(os.path.join(d, "%s.7.vtk" % name), "rb").read()
+        n_head = 9 if len(arrs) == 2 else 10
+        head = blob.split(b"\n", n_head)[:n_head]
+        assert head[0] == b"# vtk DataFile Version 2.0" and head[2] == b"BINARY"                    # L244-246
+        assert head[3] == b"DATASET STRUCTURED_POINTS" and head[4] == b"DIMENSIONS %d %d 1" % (nx, ny)
+        assert head[8] == (b"VECTORS %s double" if len(arrs) == 2 else b"SCALARS %s double 1") % name.encode()
+        body = blob[sum(len(h) + 1 for h in head):]
+        vals = np.frombuffer(body[:-1], dtype=">f8").reshape(nx * ny, -1)                             # big-endian doubles
+        assert body[-1:] == b"\n" and vals.shape[1] == (3 if len(arrs) == 2 else 1)
+        for k, a in enumerate(arrs):
+            assert (vals[:, k] == a.ravel()).all(), name
     for name, a in (("u_av", _np(t.x_average())), ("Pxy_av", _np(t.x_average_stress()))):
         m = np.loadtxt(os.path.join(d, "%s.7.dat" % name))
         assert m.shape == (ny, 2) and (m[:, 0] == np.arange(ny)).all() and (m[:, 1] == a).all()
