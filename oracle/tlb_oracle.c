@@ -10,7 +10,7 @@
  *
  * The method is an explicit iteration, so the oracle follows it step by step in the
  * paper's order and notation (PAPER Eqs. (1)-(22)); readings of silent / garbled passages
- * are the ones listed in DESIGN.md ("Readings R1..R30").  No blocking, fusion or reordering:
+ * are the ones listed in DESIGN.md ("Readings R1..R32").  No blocking, fusion or reordering:
  * every sub-step is a full sweep over the lattice writing a full array.
  *
  * Parity pins (tests/test_oracle_pins.py, all run with -m "not gpu"):

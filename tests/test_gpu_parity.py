@@ -78,6 +78,29 @@ def test_ten_step_parity(tlbmod, oracle_mod, geom, shape, taus):
     assert all(bool((p[:, solid == 1] == 0).all()) for p in pt)
 
 
+@pytest.mark.parametrize("taus", [(1.0, 1.0), (0.8, 1.4)])
+def test_unequal_wall_densities_and_temperatures_on_posts(tlbmod, oracle_mod, taus):
+    """The three readings pinned by the mutation tests of tests/test_oracle_pins.py, on the GPU side: wall densities that
+    differ between the components (L155, R9) on posts and flat walls, posts at the temperature of their own wall with
+    T_bottom != -T_top (L314, R8/R19), and a buoyancy large enough that u^(H) and u differ visibly in g^eq (L139, Eq. (18))."""
+    nx, ny = 250, 37
+    par = dict(inputs.PAPER_PHYSICS, rho_wall_A=0.9, rho_wall_B=0.2, T_bottom=1.25, T_top=0.25, T_ref=0.6, alpha_g=2e-3,
+               tau=taus[0], tau_g=taus[1])
+    solid = inputs.post_mask(nx, ny, 4, 4, 16)
+    solid[16:20, 100:103] = 1
+    o, t = _pair(tlbmod, oracle_mod, nx, ny, par, solid)
+    rA, rB, T = inputs.smooth_random_fields(nx, ny, 4, 0.75, 0.25)
+    o.set_fields(rA, rB, T)
+    t.set_fields(rA, rB, T)
+    o.step(10)
+    t.step(10)
+    assert _maxdiff(o, t) <= TOL
+    _check_fields(o, t)
+    oo, ot = o.observables(), t.observables()
+    for key in oo:
+        assert abs(ot[key] - oo[key]) <= 1e-12 * max(1.0, abs(oo[key])), key
+
+
 @pytest.mark.parametrize("physics", ["literal", "paper"])
 def test_config1_parity_and_observables(tlbmod, oracle_mod, physics):
     """BASELINE config 1 (128x64, 12 droplets r = 6, sharp interfaces + noise): 10-step parity,

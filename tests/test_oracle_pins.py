@@ -496,3 +496,104 @@ def test_obstacle_rule_is_invariant_under_the_lattice_symmetries(oracle_mod, sym
         assert np.abs(moved - b).max() < 5e-14
     fA = runs[0][0]
     assert np.abs(fA[1] - fA[3]).max() > 1e-3  # the state is not trivially symmetric itself
+
+
+# ---- pins of three readings a mutation run found unguarded ---------------------------------------------
+
+def _psi_s(rho, rho0):
+    return rho0 * (1.0 - np.exp(-rho / rho0))
+
+
+def test_wall_densities_per_species_in_the_force_stencil(oracle_mod):
+    """PAPER L155 (section 2.2.1; R9): the wall / ghost nodes carry rho_w of EACH component "respectively", so the cross
+    force on A (Eqs. (7), (8)) sees the wall density of B and the self forces (Eqs. (10)-(12)) see A's own.  Uniform fluid
+    between flat walls: every x-sum of Fig. 1(b)'s weights collapses to a row sum (exact rationals), F_x = 0, and F_y is
+    non-zero on the two rows next to each wall only:
+      row 0: -G12 psi^x_A W1 (psi^x_B - psi^x_B,w) - G11a psi^s_A W1 (psi^s_A - psi^s_A,w) - G11r psi^s_A (P1 + 2 P2)(psi^s_A - psi^s_A,w)
+      row 1: -G11r psi^s_A 2 P2 (psi^s_A - psi^s_A,w)
+    with W1 = sum_dx w(dx, 1), P1 = sum_dx p(dx, 1), P2 = sum_dx p(dx, 2); the top wall mirrors it."""
+    w = lambda dx, dy: FIG1B.get(dx * dx + dy * dy, (Fr(0), Fr(0)))[0] if max(abs(dx), abs(dy)) <= 1 else Fr(0)
+    p = lambda dx, dy: FIG1B[dx * dx + dy * dy][1]
+    W1 = float(sum(w(dx, 1) for dx in range(-1, 2)))
+    P1 = float(sum(p(dx, 1) for dx in range(-2, 3)))
+    P2 = float(sum(p(dx, 2) for dx in range(-2, 3)))
+    assert (W1, P1) == (float(Fr(1, 6)), float(Fr(4, 63) + Fr(8, 135) + Fr(4, 945)))
+    nx, ny = 6, 9
+    par = dict(PAPER_FORCES, rho_wall_A=0.9, rho_wall_B=0.2)
+    rho = dict(A=1.3, B=0.45)
+    o = oracle_mod.Oracle(nx, ny, **par)
+    o.set_fields(np.full((ny, nx), rho["A"]), np.full((ny, nx), rho["B"]), np.zeros((ny, nx)))
+    F = dict(zip("AB", o.forces()))
+    r0 = par["rho0"]
+    for me, other, Ga, Gr in (("A", "B", par["G11a"], par["G11r"]), ("B", "A", par["G22a"], par["G22r"])):
+        px, px_o, px_ow = rho[me] / r0, rho[other] / r0, par["rho_wall_" + other] / r0
+        ps, ps_w = _psi_s(rho[me], r0), _psi_s(par["rho_wall_" + me], r0)
+        row0 = -par["G12"] * px * W1 * (px_o - px_ow) - Ga * ps * W1 * (ps - ps_w) - Gr * ps * (P1 + 2 * P2) * (ps - ps_w)
+        row1 = -Gr * ps * 2 * P2 * (ps - ps_w)
+        expect = np.zeros(ny)
+        expect[0], expect[1], expect[-1], expect[-2] = row0, row1, -row0, -row1
+        assert abs(row0) > 1e-4 and abs(row1) > 1e-6
+        assert np.abs(F[me][1] - expect[:, None]).max() <= 1e-15, me
+        assert np.abs(F[me][0]).max() <= 1e-16, me
+    # exact fixed point: a fluid at the wall densities feels no force anywhere, obstacles included
+    nx, ny = 32, 24
+    solid = inputs.post_mask(nx, ny, 4, 4, 16)
+    solid[10:13, 7:9] = 1
+    o = oracle_mod.Oracle(nx, ny, **par)
+    o.set_solid(solid)
+    o.set_fields(np.full((ny, nx), 0.9), np.full((ny, nx), 0.2), np.zeros((ny, nx)))
+    for Fl in o.forces():
+        assert np.abs(Fl).max() <= 1e-15
+
+
+def test_posts_carry_the_temperature_of_their_wall(oracle_mod):
+    """PAPER L314 (section 3.2.3: Tdown / Tup) with BASELINE config 4 "wall temperature on posts" (R8, R19): a post of the
+    bottom wall is at T_bottom, one of the top wall at T_top.  Pure conduction (G = 0, alpha g = 0, fluid at rest) between
+    walls with aligned posts: the problem is antisymmetric about the mid-plane, T(x, y) + T(x, ny-1-y) = T_b + T_t at
+    all times (posts at one temperature on both walls would break it), and a bottom post heats the fluid above it beyond
+    the smooth-wall conduction profile (a post at any lower temperature would not)."""
+    nx, ny, Tb, Tt = 16, 16, 1.25, 0.25
+    solid = inputs.post_mask(nx, ny, 4, 4, 8)
+    assert np.array_equal(solid, solid[::-1]) and solid[:4].any() and not solid[4:-4].any()
+    o = oracle_mod.Oracle(nx, ny, tau=1.0, tau_g=0.8, T_bottom=Tb, T_top=Tt, T_ref=0.75)
+    o.set_solid(solid)
+    lin = Tb - (Tb - Tt) * (np.arange(ny) + 0.5) / ny
+    o.set_fields(np.full((ny, nx), 0.6), np.full((ny, nx), 0.4), lin[:, None].repeat(nx, 1))
+    o.step(4000)
+    rA, rB, u, T = o.fields()
+    fluid = solid == 0
+    assert np.abs(u).max() < 1e-15
+    assert np.abs((T + T[::-1])[fluid] - (Tb + Tt)).max() <= 1e-12
+    o.step(1)
+    assert np.abs(o.fields()[3] - T).max() < 1e-12      # steady
+    above = [x for x in range(nx) if solid[3, x]]       # columns of the bottom posts; their top face is at y = 3.5
+    assert len(above) == 8
+    # next to the face the temperature is within half a cell's gradient of T_bottom, far above the smooth-wall value
+    assert (T[4, above] > Tb - 0.5 * (Tb - Tt) / (ny - 8) * 1.5).all() and (T[4, above] > lin[4] + 0.15).all()
+    assert (T[fluid] <= Tb + 1e-12).all() and (T[fluid] >= Tt - 1e-12).all()
+    notch = [x for x in range(nx) if not solid[0, x]]
+    assert (T[0, notch] > T[ny // 2 - 1, notch]).all()
+
+
+def test_thermal_equilibrium_is_taken_at_the_hydrodynamic_velocity(oracle_mod):
+    """Eqs. (16), (18) with L139: g^eq is evaluated at u^(H) = u + F / (2 rho), not at the bare u of
+    Eq. (5).  One step at tau_g = 1 relaxes g onto g^eq exactly, so g_i(x + c_i, 1) = w_i T [1 + 3 c_i.u^(H) +
+    4.5 (c_i.u^(H))^2 - 1.5 |u^(H)|^2] with u^(H) = (rho_A U_A + rho_B U_B) / rho + (alpha g / 2)(T - T_ref) e_y in closed
+    form (G = 0: buoyancy, Eq. (22), is the only force).  With u in place of u^(H) the populations differ by
+    3 w_i T (alpha g / 2)(T - T_ref) ~ 1e-3."""
+    nx, ny, ag, Tref = 12, 10, 3e-2, 0.2
+    rA, rB, T, UA, UB = _flow_state(nx, ny, 5)
+    o = oracle_mod.Oracle(nx, ny, tau=0.9, tau_g=1.0, periodic_y=1, alpha_g=ag, T_ref=Tref)
+    o.set_populations(_linear_pops(rA, *UA), _linear_pops(rB, *UB), _linear_pops(T, 0.3 * UA[0], -0.2 * UB[1]))
+    o.step(1)
+    g1 = o.get_populations()[2]
+    rho = rA + rB
+    uHx = (rA * UA[0] + rB * UB[0]) / rho
+    uHy = (rA * UA[1] + rB * UB[1]) / rho + 0.5 * ag * (T - Tref)
+    assert np.abs(0.5 * ag * (T - Tref)).max() > 5e-3
+    cx, cy = _CX[:, 0, 0], _CY[:, 0, 0]
+    for i in range(9):
+        cu = cx[i] * uHx + cy[i] * uHy
+        geq = _WQ[i, 0, 0] * T * (1 + 3 * cu + 4.5 * cu * cu - 1.5 * (uHx * uHx + uHy * uHy))
+        moved = np.roll(np.roll(geq, cy[i], axis=0), cx[i], axis=1)   # g_i(x + c_i, t + 1) = g*_i(x, t)
+        assert np.abs(g1[i] - moved).max() <= 1e-15, i
