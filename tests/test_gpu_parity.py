@@ -268,15 +268,16 @@ def test_full_size_windows_config4(tlbmod, oracle_mod, tau):
     """tau = 1 runs the kernel instantiation bench.py times; tau = 0.9 the general one (four slots, the populations
     relaxed and not only their moments) in the same launch configuration.
     BASELINE config 4 at full size (4096x2048, posts, 4000 droplets) in the launch configuration bench.py
-    times: 3 steps on the GPU, compared with the oracle on windows it can compute in seconds.  A site after
-    n steps depends on initial data within 3n cells (2-cell force stencil + 1 cell of streaming per step), so
-    an oracle run on a window is exact farther than 3n cells from the window's artificial edges.  Windows:
-    bottom wall + posts, top wall + posts, the periodic seam in x, a strip edge (x = 128 k) crossing a
-    segment edge, and a bulk window."""
+    times: 10 steps on the GPU (the north_star's count), compared with the oracle on windows it can compute in
+    seconds.  A site after n steps depends on initial data within 3n cells (2-cell force stencil + 1 cell of
+    streaming per step), so an oracle run on a window is exact farther than 3n cells from the window's artificial
+    edges (margin 3n + 2 = 32).  Windows: bottom wall + posts, top wall + posts, the periodic seam in x, a strip edge
+    (x = 128 k) crossing a segment edge, a strip edge crossing TWO consecutive segment edges, and a bulk window."""
     import torch
     cfg = inputs.config(4)
     cfg["params"] = dict(cfg["params"], tau=tau, tau_g=tau)
-    nx, ny, steps, m = cfg["nx"], cfg["ny"], 3, 12
+    nx, ny, steps = cfg["nx"], cfg["ny"], 10
+    m = 3 * steps + 2
     solid, rA, rB, T = inputs.make_config_inputs(cfg)
     t = tlbmod.TLB(nx, ny, params=tlbmod.params_from_config(cfg))
     t.init(cfg["seed"])
@@ -284,13 +285,14 @@ def test_full_size_windows_config4(tlbmod, oracle_mod, tau):
     pops = t.get_populations()
     ob = t.observables()
     assert all(np.isfinite(v) for v in ob.values())
-    seg = t.seg_rows()  # rows per CTA segment, read back from the library; the "edges" window straddles y = seg and x = 128
-    assert 30 < seg < ny - 30
-    windows = [("bottom", np.arange(1000, 1200), np.arange(0, 48), "wall_bottom"),
-               ("top", np.arange(3000, 3200), np.arange(ny - 48, ny), "wall_top"),
-               ("seam", np.r_[np.arange(nx - 80, nx), np.arange(0, 80)], np.arange(900, 960), "bulk"),
-               ("edges", np.arange(128 - 70, 128 + 70), np.arange(seg - 30, seg + 30), "bulk"),
-               ("bulk", np.arange(2000, 2150), np.arange(1500, 1560), "bulk")]
+    seg = t.seg_rows()  # rows per CTA segment, read back from the library; the "edges" windows straddle y = 4 seg (and 5 seg)
+    assert 30 < seg and 5 * seg + 60 < ny
+    windows = [("bottom", np.arange(1000, 1200), np.arange(0, 80), "wall_bottom"),
+               ("top", np.arange(3000, 3200), np.arange(ny - 80, ny), "wall_top"),
+               ("seam", np.r_[np.arange(nx - 100, nx), np.arange(0, 100)], np.arange(900, 1010), "bulk"),
+               ("edges", np.arange(128 - 100, 128 + 100), np.arange(4 * seg - 55, 4 * seg + 55), "bulk"),
+               ("two_edges", np.arange(128 * 9 - 100, 128 * 9 + 100), np.arange(4 * seg - 45, 5 * seg + 45), "bulk"),
+               ("bulk", np.arange(2000, 2200), np.arange(1500, 1610), "bulk")]
     for name, xs, ys, kind in windows:
         sub = np.ix_(ys, xs)
         par = dict(cfg["params"], periodic_y=1 if kind == "bulk" else 0)
