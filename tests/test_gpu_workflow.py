@@ -232,6 +232,11 @@ def test_bench_json_contract(tlbmod):
     assert r["bound"] == "hbm" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12
     c = d["cpu_baseline"]
     assert c["kind"] == "oracle" and c["cores"] == 1 and c["value"] > 0 and "sample" in c
-    e = d["e2e"]
-    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 3 * 8 * 128 * 64 and e["d2h_bytes_per_step"] == 32
+    e = d["e2e"]   # the loop that returns the step's result: three field planes in, five out
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == 3 * 8 * 128 * 64 and e["d2h_bytes_per_step"] == 5 * 8 * 128 * 64
+    assert d["e2e_observables"]["d2h_bytes_per_step"] == 32 and d["e2e_observables"]["value"] > e["value"]
+    sus = r["sustained"]   # the config's own step count (config 1: 1000), timed after the K-step region
+    assert sus["steps"] == 1000 and sus["ms_per_step"] > 0 and sus["frac"] > 0 and "clocks" in sus
+    assert d["droplet_analysis"]["n_droplets"] == 12 and d["droplet_analysis"]["whole_analysis_lb_steps"] > 0
+    assert d["scaling"] == "strong"
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
