@@ -181,6 +181,22 @@ class DistributedSlab(Slab):
         super().__init__(nx, ny, dist.get_rank(), dist.get_world_size(), params=params, device=device, **overrides)
         self.comm_stream = torch.cuda.Stream(device=self.t.device)
         self.packed, self.arrived = torch.cuda.Event(), torch.cuda.Event()
+        # A gloo group cannot send device memory: the faces are then staged through host tensors (what a node without
+        # GPU-direct transport would do, and what lets two ranks share ONE GPU in the tests).  NCCL reads and writes the
+        # population buffers directly.
+        self.host_staged = dist.get_backend() == "gloo"
+
+    def _exchange(self):
+        """Runs on the side stream, after the edge rows of this step: move the faces to / from the neighbours."""
+        if not self.host_staged:
+            exchange(self.dist, self.send, self.recv, self.lo, self.hi, self.rank)
+            return
+        send_h = [None if s is None else s.cpu() for s in self.send]          # synchronous copies on the side stream
+        recv_h = [None if r is None else self.torch.empty_like(r, device="cpu") for r in self.recv]
+        exchange(self.dist, send_h, recv_h, self.lo, self.hi, self.rank)
+        for r, h in zip(self.recv, recv_h):
+            if r is not None:
+                r.copy_(h)
 
     def step(self, n=1):
         torch, main = self.torch, self.t.stream
@@ -196,7 +212,7 @@ class DistributedSlab(Slab):
             self.t.slab_step_interior()              # overlaps the exchange below
             with torch.cuda.stream(self.comm_stream):
                 self.comm_stream.wait_event(self.packed)
-                exchange(self.dist, self.send, self.recv, self.lo, self.hi, self.rank)
+                self._exchange()
                 self.arrived.record(self.comm_stream)
             main.wait_event(self.arrived)
             self.end_step()
@@ -205,5 +221,10 @@ class DistributedSlab(Slab):
         """dict(mass_A, mass_B, E, Nu) of the whole lattice: all-reduce of the slabs' six sums."""
         sums = self.t.observable_sums()
         if self.world > 1:
-            self.dist.all_reduce(sums, op=self.dist.ReduceOp.SUM)
+            if self.host_staged:
+                host = sums.cpu()
+                self.dist.all_reduce(host, op=self.dist.ReduceOp.SUM)
+                sums.copy_(host)
+            else:
+                self.dist.all_reduce(sums, op=self.dist.ReduceOp.SUM)
         return self.t.observables_from_sums(sums)

@@ -1,6 +1,8 @@
 """GPU parity, round 2: y-slabs against one handle and the oracle, the stress field, the droplet labelling, the
 one-pass observables, and BASELINE.json's configs 2, 3, 5 (+ the fp32-storage study) at full size.  Everything goes
 through the C ABI; expected values come from the CPU oracle on the same seeded inputs."""
+import os
+
 import numpy as np
 import pytest
 
@@ -423,3 +425,67 @@ def test_distributed_slab_world1_nccl(tlbmod):
             assert abs(ob_s[k] - ob_1[k]) <= 1e-13 * max(1.0, abs(ob_1[k]))
     finally:
         dist.destroy_process_group()
+
+
+def _two_rank_worker(rank, port, geom, taus, out_dir):
+    """One of two processes sharing cuda:0, each with its own slab of the lattice, talking over gloo."""
+    import torch
+    import torch.distributed as dist
+    from paper_2109_12565_b200 import slabs as S
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=2)
+    try:
+        nx, ny, par, solid, (rA, rB, T) = _two_rank_case(geom, taus)
+        s = S.DistributedSlab(nx, ny, device="cuda:0", **par)
+        assert s.host_staged and s.world == 2 and (s.lo == s.hi == 1 - rank if par["periodic_y"] else True)
+        s.set_solid(solid)
+        s.set_fields(rA, rB, T)
+        s.step(10)
+        torch.cuda.synchronize()
+        ob = s.observables()   # all-reduce of the six sums over the two ranks
+        pops = [s.owned(p).cpu().numpy() for p in s.t.get_populations()]
+        np.savez(os.path.join(out_dir, "rank%d.npz" % rank), fA=pops[0], fB=pops[1], g=pops[2], y0=s.y0, y1=s.y1,
+                 ob=np.array([ob[k] for k in ("mass_A", "mass_B", "E", "Nu")]))
+    finally:
+        dist.destroy_process_group()
+
+
+def _two_rank_case(geom, taus):
+    nx, ny = 200, 46
+    per = 1 if geom == "periodic_y_mask" else 0
+    par = dict(inputs.PAPER_PHYSICS, alpha_g=1e-4, periodic_y=per, tau=taus[0], tau_g=taus[1])
+    if per:
+        solid = (inputs.uniform(8, 9, np.arange(nx * ny)).reshape(ny, nx) < 0.1).astype(np.uint8)
+    else:
+        solid = inputs.post_mask(nx, ny, 4, 4, 16)
+        solid[ny // 2 - 2:ny // 2 + 3, 30:37] = 1   # an obstacle that straddles the face between the two slabs
+    return nx, ny, par, solid, inputs.smooth_random_fields(nx, ny, 2, 0.5, -0.5)
+
+
+@pytest.mark.parametrize("geom,taus", [("posts", (1.0, 1.0)), ("periodic_y_mask", (1.0, 1.0)), ("periodic_y_mask", (0.9, 0.8))])
+def test_distributed_slab_two_ranks_on_one_gpu(tlbmod, geom, taus, tmp_path):
+    """slabs.DistributedSlab with TWO real ranks: two processes share cuda:0, each owns half of the lattice, and the faces
+    travel between them over a gloo group (staged through host tensors; nothing on the GPU waits for the other process:
+    every wait is a host wait).  This runs what the world-size-1 test cannot: the exchange with a real peer, both
+    directions to the same peer on a y-periodic lattice (lo == hi), the side stream and its two events, and the
+    all-reduced observables.  After 10 steps the owned rows are bit for bit those of one handle on the whole lattice."""
+    import socket
+    import torch.multiprocessing as mp
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    mp.spawn(_two_rank_worker, args=(port, geom, taus, str(tmp_path)), nprocs=2, join=True)
+    nx, ny, par, solid, (rA, rB, T) = _two_rank_case(geom, taus)
+    one = tlbmod.TLB(nx, ny, **par)
+    one.set_solid(solid)
+    one.set_fields(rA, rB, T)
+    one.step(10)
+    ref = [_np(p) for p in one.get_populations()]
+    ob_1 = one.observables()
+    parts = [np.load(os.path.join(str(tmp_path), "rank%d.npz" % r)) for r in range(2)]
+    assert int(parts[0]["y0"]) == 0 and int(parts[0]["y1"]) == int(parts[1]["y0"]) and int(parts[1]["y1"]) == ny
+    for k, name in enumerate(("fA", "fB", "g")):
+        assert np.array_equal(ref[k], np.concatenate([p[name] for p in parts], axis=-2)), name
+    for p in parts:   # both ranks hold the same all-reduced observables
+        for v, key in zip(p["ob"], ("mass_A", "mass_B", "E", "Nu")):
+            assert abs(v - ob_1[key]) <= 1e-13 * max(1.0, abs(ob_1[key])), key
