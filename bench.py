@@ -133,7 +133,7 @@ def time_oracle(cfg, solid, rA, rB, T, steps):
 
 def slab_of(cfg, rows):
     """A full-width slab of `rows` rows of the workload (walls, posts, droplets, same physics)."""
-    from paper_2109_12565_b200 import inputs
+    import inputs
     if rows >= cfg["ny"]:
         return cfg, inputs.make_config_inputs(cfg)
     c = dict(cfg, ny=rows)
@@ -151,7 +151,7 @@ def run_reference(args, rank):
     host cores, each step a bounded slab of the workload sized so the run ends within minutes."""
     if rank != 0:
         return
-    from paper_2109_12565_b200 import inputs
+    import inputs
     cfg = inputs.config(args.config)
     budget_sites = 90e6  # about 90 s at ~1 MLUPS
     rows = int(budget_sites / max(1, args.steps + args.warmup) / cfg["nx"])
@@ -181,7 +181,8 @@ def run_reference(args, rank):
 def run_ours(args, rank, world):
     import torch
     import torch.distributed as dist
-    from paper_2109_12565_b200 import binding, inputs, replicas
+    from paper_2109_12565_b200 import binding, replicas
+    import inputs
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
@@ -404,7 +405,8 @@ def run_slabs(args, rank, world, local):
     """N > 1: y-slab decomposition, one process per GPU."""
     import torch
     import torch.distributed as dist
-    from paper_2109_12565_b200 import binding, inputs, replicas, slabs
+    from paper_2109_12565_b200 import binding, replicas, slabs
+    import inputs
 
     dev = "cuda:%d" % local
     dist.init_process_group("nccl", device_id=torch.device(dev))

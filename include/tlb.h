@@ -50,11 +50,14 @@
  *   whole lattice; state-setting calls take the halo rows from the caller's arrays, output calls write the
  *   owned rows only.  One time step is
  *       tlb_slab_step_edges     fused kernel on the 3 owned rows next to each halo face
- *       tlb_halo_pack(face)     those rows of all 27 planes -> a contiguous buffer of tlb_halo_bytes
  *       tlb_slab_step_interior  fused kernel on the remaining owned rows (overlaps the exchange)
- *       ... the caller moves each packed buffer to the neighbour across that face (NCCL, peer copy) ...
- *       tlb_halo_unpack(face)   neighbour's buffer -> the halo rows beyond `face`
+ *       ... the caller moves the 3 edge rows of each face into the neighbour's halo rows ...
  *       tlb_slab_step_finish    boundary kernel over every solid node of the local lattice; state advances
+ *   The default transport is zero-copy: the 27 plane rows of a lattice row lie next to one another, so the rows to
+ *   export and the halo rows to fill are each ONE contiguous block of tlb_halo_bytes inside the population buffer, and
+ *   tlb_halo_region(face, which) returns their device pointers for NCCL send / recv, a peer copy or a peer-mapped
+ *   store to read and write directly.  tlb_halo_pack(face) / tlb_halo_unpack(face) copy the same rows to / from a
+ *   separate buffer for transports that want one (the staged alternative; both give bit-identical states).
  *   (3 rows: the pull of the 2 force-stencil rows beyond a face reaches one row further.)  The result is bit
  *   for bit that of one handle on the whole lattice.  tlb_observable_sums gives a slab's share of the six
  *   sums behind tlb_observables; after an all-reduce tlb_observables_from_sums finishes them.
@@ -136,7 +139,7 @@ int tlb_seg_rows(const tlb_handle* h);
 
 /* Seeded initial state of the input recipe: structured posts from params, n_droplets
  * discs by random sequential addition, +noise, linear T profile (L314), populations at rest
- * equilibrium f = w rho, g = w T (R14).  Bit-identical to paper_2109_12565_b200/inputs.py. */
+ * equilibrium f = w rho, g = w T (R14).  Bit-identical to inputs/__init__.py (the seeded generators next to oracle/). */
 int tlb_init(tlb_handle* h, uint64_t seed);
 
 /* The same with the paper's own droplet arrangement ("droplet initialisation = 1", L266: "we initialise the soft domains

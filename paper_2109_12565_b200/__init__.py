@@ -1,9 +1,9 @@
 """B200-native thermal two-component D2Q9 lattice-Boltzmann step (TLBfind, arXiv 2109.12565).
 
-`inputs` (seeded synthetic workloads) imports eagerly; the CUDA binding loads the C-ABI shared
-library on first use and fails loudly if it is missing -- there is no CPU fallback.
+The CUDA binding loads the C-ABI shared library on first use and fails loudly if it is missing -- there is no
+CPU fallback.  The package holds the product only: the seeded input generators that feed both it and the oracle in the
+tests live in the top-level `inputs` module.
 """
-from . import inputs  # noqa: F401
 
 
 def __getattr__(name):

@@ -110,7 +110,7 @@ __global__ void pad_mask_kernel(const Dev d, uint8_t* __restrict__ solidp) {
   solidp[k] = v;
 }
 
-// ---- seeded input recipe (must reproduce paper_2109_12565_b200/inputs.py bit for bit) ----
+// ---- seeded input recipe (must reproduce inputs/__init__.py bit for bit) ----
 __device__ __forceinline__ double uniform01(uint64_t seed, uint64_t stream, uint64_t k) {
   uint64_t z = seed + 0x9E3779B97F4A7C15ull * ((stream << 40) + k + 1ull);
   z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;

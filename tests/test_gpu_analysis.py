@@ -4,8 +4,7 @@ the same seeded inputs.  Integer outputs must be bit-identical."""
 import numpy as np
 import pytest
 
-from paper_2109_12565_b200 import inputs
-
+import inputs
 pytestmark = pytest.mark.gpu
 
 

@@ -5,8 +5,7 @@ after 10 steps; integer / byte work (masks, seeded initial state) bit-exact.
 import numpy as np
 import pytest
 
-from paper_2109_12565_b200 import inputs
-
+import inputs
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-12
@@ -138,7 +137,7 @@ def test_config4_geometry_small(tlbmod, oracle_mod):
 
 def test_init_matches_input_recipe_bitwise(tlbmod):
     """tlb_init(seed) implements DESIGN.md's input recipe natively: mask, densities and temperature
-    are bit-identical to paper_2109_12565_b200/inputs.py."""
+    are bit-identical to inputs/__init__.py."""
     for idx, phys in ((1, "literal"), (2, "paper")):
         cfg = inputs.config(idx, phys)
         solid, rA, rB, T = inputs.make_config_inputs(cfg)

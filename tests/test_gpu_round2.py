@@ -6,8 +6,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2109_12565_b200 import inputs
-
+import inputs
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-12

@@ -310,7 +310,7 @@ def test_voronoi_at_is_voronoi_on_listed_sites(oracle_mod):
 
 def test_rough_walls_rectangles_are_the_post_mask(oracle_mod):
     """alpha = 0: "a simple rectangular-shape roughness" (L366) = the structured posts of the headline config."""
-    from paper_2109_12565_b200 import inputs
+    import inputs
     for nx, ny, w, h, lam in ((64, 24, 4, 4, 16), (150, 40, 10, 7, 30), (33, 12, 5, 3, 11)):
         assert (oracle_mod.rough_walls(nx, ny, 1, 1, w, h, lam, 0.0, 0) == inputs.post_mask(nx, ny, w, h, lam)).all()
         only_down = oracle_mod.rough_walls(nx, ny, 0, 1, w, h, lam, 0.0, 1)
@@ -366,7 +366,7 @@ def test_velocity_perturbation_closed_form(oracle_mod):
 
 def test_honeycomb_centres_arrangement():
     """L266: honeycomb structure of ndx x ndy droplets: equal spacing along x, rows offset by half a spacing."""
-    from paper_2109_12565_b200 import inputs
+    import inputs
     nx, ny, ndx, ndy = 120, 104, 6, 6
     c = inputs.honeycomb_centres(nx, ny, ndx, ndy)
     assert c.shape == (36, 2)

@@ -10,8 +10,7 @@ from fractions import Fraction as Fr
 import numpy as np
 import pytest
 
-from paper_2109_12565_b200 import inputs
-
+import inputs
 GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
 
 # Fig. 1(b), typed from the paper: |c|^2 -> (w, p)

@@ -12,8 +12,7 @@ P_xy has no formula in the paper, so it is pinned by what mechanics fixes:
 import numpy as np
 import pytest
 
-from paper_2109_12565_b200 import inputs
-
+import inputs
 CX = np.array([0, 1, 0, -1, 0, 1, -1, -1, 1])[:, None, None]
 CY = np.array([0, 0, 1, 0, -1, 1, 1, -1, -1])[:, None, None]
 WQ = np.array([4 / 9] + [1 / 9] * 4 + [1 / 36] * 4)[:, None, None]

@@ -20,7 +20,8 @@ def _worker(rank, world, port, out):
     sys.path.insert(0, ROOT)
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     import torch.distributed as dist
-    from paper_2109_12565_b200 import inputs, replicas
+    from paper_2109_12565_b200 import replicas
+    import inputs
     dist.init_process_group("gloo", rank=rank, world_size=world)
     cfg = inputs.config(1)
     seed = replicas.rank_seed(cfg["seed"], rank)

@@ -14,9 +14,7 @@ import ctypes
 import numpy as np
 import pytest
 
-from paper_2109_12565_b200 import inputs
-
-
+import inputs
 def _flipped_grid(cols, rows, n_flips, seed):
     """Link lists of a triangulated cols x rows grid (past) and of the same grid with n_flips diagonals flipped and the
     droplets renumbered (now); map[k] = past index of present droplet k, one droplet of a flipped square unmatched."""
