@@ -182,12 +182,15 @@ int tlb_read_checkpoint(tlb_handle* h, const char* dir, int32_t index);
  *   TLB_OUT_TEMPERATURE  temperature.<i>.dat                              T
  *   TLB_OUT_VELOCITY     veloconf.<i>.dat, u_av.<i>.dat                   u^(H) (two columns), its x-average of u_x per row
  *   TLB_OUT_STRESS       Ptot_xy.<i>.dat, Pxy_av.<i>.dat                  P_xy (R21), its x-average per row
+ *   TLB_OUT_ENERGY       timeEnergy.dat                                   one line "<i> E" APPENDED per call (L248: the kinetic
+ *                                                                         energy E of tlb_observables "appended every nout
+ *                                                                         energy steps"; pass the time step as index)
  * The paper names the files, not their format; reading R31: ASCII, one line "x y value" per site (velocity: "x y u_x
  * u_y"; the averages: "y value"), x fastest, a blank line after every lattice row, numbers printed with 17 significant
  * digits (they read back to the same doubles).  vtk != 0 adds <name>.<i>.vtk for the fields ("binary VTK 2.0", L244-246:
  * legacy "# vtk DataFile Version 2.0" header, BINARY, STRUCTURED_POINTS, one SCALARS / VECTORS array of big-endian doubles;
  * "write vtk file" of Table C.9).  Synchronises; TLB_EIO on a file error; TLB_EINVAL on slab handles. */
-enum { TLB_OUT_DENSITY = 1, TLB_OUT_TEMPERATURE = 2, TLB_OUT_VELOCITY = 4, TLB_OUT_STRESS = 8 };
+enum { TLB_OUT_DENSITY = 1, TLB_OUT_TEMPERATURE = 2, TLB_OUT_VELOCITY = 4, TLB_OUT_STRESS = 8, TLB_OUT_ENERGY = 16 };
 int tlb_write_fields(tlb_handle* h, const char* dir, int32_t index, int32_t what, int32_t vtk);
 
 /* Arbitrary obstacle mask [ny][nx], non-zero = solid (flag field, L286).  Resets the state. */

@@ -322,7 +322,7 @@ class TLB:
     def write_checkpoint(self, directory, index=0):
         self._chk(self.lib.tlb_write_checkpoint(self.h, os.fsencode(directory), int(index)))
 
-    OUT_DENSITY, OUT_TEMPERATURE, OUT_VELOCITY, OUT_STRESS = 1, 2, 4, 8
+    OUT_DENSITY, OUT_TEMPERATURE, OUT_VELOCITY, OUT_STRESS, OUT_ENERGY = 1, 2, 4, 8, 16
 
     def write_fields(self, directory, index=0, what=15, vtk=False):
         """The field files of Tables C.9 / C.10 (firstdensity.<i>.dat, ..., Pxy_av.<i>.dat; reading R31)."""

@@ -715,7 +715,7 @@ static bool write_vtk(const std::string& path, const char* name, int nx, int ny,
 }
 
 int tlb_write_fields(tlb_handle* h, const char* dir, int32_t index, int32_t what, int32_t vtk) {
-  if (!h || !dir || what < 0 || what > 15) return TLB_EINVAL;
+  if (!h || !dir || what < 0 || what > 31) return TLB_EINVAL;
   if (h->slab) return TLB_EINVAL;
   if (!h->has_state || h->step_open) return TLB_ESTATE;
   const int nx = h->d.nx, ny = h->d.ny;
@@ -749,6 +749,14 @@ int tlb_write_fields(tlb_handle* h, const char* dir, int32_t index, int32_t what
     if (!field("Ptot_xy", a.data(), nullptr)) return TLB_EIO;
     if ((rc = tlb_x_average_stress_host(h, b.data())) != TLB_OK) return rc;
     if (!write_profile(base + "Pxy_av" + tag + ".dat", ny, b.data())) return TLB_EIO;
+  }
+  if (what & TLB_OUT_ENERGY) {  // timeEnergy.dat (L248): one line per call, appended
+    double o4[4];
+    if ((rc = tlb_observables_host(h, o4)) != TLB_OK) return rc;
+    FILE* f = std::fopen((base + "timeEnergy.dat").c_str(), "a");
+    if (!f) return TLB_EIO;
+    const bool ok = std::fprintf(f, "%d %.17g\n", (int)index, o4[2]) >= 0;
+    if (std::fclose(f) != 0 || !ok) return TLB_EIO;
   }
   return TLB_OK;
 }

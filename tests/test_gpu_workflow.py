@@ -201,6 +201,15 @@ def test_write_fields_round_trip(tlbmod, tmp_path):
     # only what was asked for is written
     t.write_fields(d, 8, what=t.OUT_TEMPERATURE)
     assert sorted(f for f in os.listdir(d) if ".8." in f) == ["temperature.8.dat"]
+    # timeEnergy.dat (L248): one "<index> E" line appended per call, E the observable, 17 digits
+    assert not os.path.exists(os.path.join(d, "timeEnergy.dat"))
+    e25 = t.observables()["E"]
+    t.write_fields(d, 25, what=t.OUT_ENERGY)
+    t.step(5)
+    t.write_fields(d, 30, what=t.OUT_ENERGY)
+    rows = np.loadtxt(os.path.join(d, "timeEnergy.dat"))
+    assert rows.shape == (2, 2) and (rows[:, 0] == [25, 30]).all()
+    assert rows[0, 1] == e25 and rows[1, 1] == t.observables()["E"] and e25 > 0
     with pytest.raises(tlbmod.TLBError) as e:
         t.write_fields(os.path.join(d, "missing"), 9)
     assert e.value.code == tlbmod.TLB_EIO
